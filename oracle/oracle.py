@@ -1,0 +1,191 @@
+"""ctypes front-end of the fp64 CPU oracle (oracle/sap_oracle.cpp).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference leg may import this.  It imports nothing
+from paper_2606_30460_b200 (the CUDA path) and shares no code with it.
+
+Arrays are numpy; Q/K/V/dO are float32 arrays holding bf16-exact values
+(`tensor.float().numpy()`); every result is float64.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sap_oracle.cpp")
+_LIB = os.path.join(_HERE, "libsap_oracle.so")
+
+SKIP, FULL, DIAG = 0, 1, 2
+ITEM_FIELDS = ("q_chunk", "kv_chunk", "doc_lo", "doc_hi", "mask_kind", "step",
+               "q_begin", "q_end", "kv_begin", "kv_end")
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ (x86-64-v3 so the .so also runs on the GPU box's host)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["g++", "-O3", "-march=x86-64-v3", "-std=c++17", "-fopenmp", "-fPIC", "-shared",
+               "-fno-fast-math", "-o", _LIB, _SRC]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        _lib.sap_oracle_num_threads.restype = ctypes.c_int
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().sap_oracle_num_threads())
+
+
+def _f32(a):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    return a, a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _i32(a):
+    a = np.ascontiguousarray(a, dtype=np.int32)
+    return a, a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _i64_or_null(a):
+    if a is None:
+        return None, ctypes.c_void_p(0), 0
+    a = np.ascontiguousarray(a, dtype=np.int64)
+    return a, a.ctypes.data_as(ctypes.c_void_p), a.shape[0]
+
+
+def _dims(q, k):
+    N, Hq, d = q.shape
+    Hkv = k.shape[1]
+    return N, Hq, Hkv, d
+
+
+def attn_fwd(q, k, v, cu_seqlens, scale: float, rows: Optional[Sequence[int]] = None):
+    """Exact per-document causal attention.  Returns (O [n_rows,Hq,d], LSE [n_rows,Hq])."""
+    q, qp = _f32(q); k, kp = _f32(k); v, vp = _f32(v)
+    cu, cup = _i32(cu_seqlens)
+    N, Hq, Hkv, d = _dims(q, k)
+    rows_a, rp, nr = _i64_or_null(rows)
+    if rows is None:
+        nr = N
+    o = np.empty((nr, Hq, d), dtype=np.float64)
+    lse = np.empty((nr, Hq), dtype=np.float64)
+    rc = lib().sap_oracle_fwd(qp, kp, vp, cup, ctypes.c_int(len(cu) - 1), ctypes.c_int64(N),
+                              ctypes.c_int(Hq), ctypes.c_int(Hkv), ctypes.c_int(d),
+                              ctypes.c_double(scale), rp, ctypes.c_int64(nr),
+                              o.ctypes.data_as(ctypes.c_void_p), lse.ctypes.data_as(ctypes.c_void_p))
+    if rc != 0:
+        raise ValueError(f"sap_oracle_fwd: bad arguments ({rc})")
+    return o, lse
+
+
+def attn_partial(q, k, v, cu_seqlens, scale: float, q_begin: int, q_end: int, kv_begin: int, kv_end: int):
+    """Partial attention of one work item.  Returns (O [rows,Hq,d], LSE [rows,Hq]); -inf/0 for empty rows."""
+    q, qp = _f32(q); k, kp = _f32(k); v, vp = _f32(v)
+    cu, cup = _i32(cu_seqlens)
+    N, Hq, Hkv, d = _dims(q, k)
+    nr = q_end - q_begin
+    o = np.empty((nr, Hq, d), dtype=np.float64)
+    lse = np.empty((nr, Hq), dtype=np.float64)
+    rc = lib().sap_oracle_partial(qp, kp, vp, cup, ctypes.c_int(len(cu) - 1), ctypes.c_int64(N),
+                                  ctypes.c_int(Hq), ctypes.c_int(Hkv), ctypes.c_int(d),
+                                  ctypes.c_double(scale), ctypes.c_int64(q_begin), ctypes.c_int64(q_end),
+                                  ctypes.c_int64(kv_begin), ctypes.c_int64(kv_end),
+                                  o.ctypes.data_as(ctypes.c_void_p), lse.ctypes.data_as(ctypes.c_void_p))
+    if rc != 0:
+        raise ValueError("sap_oracle_partial: bad arguments")
+    return o, lse
+
+
+def lse_merge(o_a, lse_a, o_b, lse_b):
+    """Exact merge of two partials over disjoint key sets.  o_* [...,d], lse_* [...]."""
+    o_a = np.ascontiguousarray(o_a, dtype=np.float64); o_b = np.ascontiguousarray(o_b, dtype=np.float64)
+    lse_a = np.ascontiguousarray(lse_a, dtype=np.float64); lse_b = np.ascontiguousarray(lse_b, dtype=np.float64)
+    d = o_a.shape[-1]
+    n = lse_a.size
+    o = np.empty_like(o_a); lse = np.empty_like(lse_a)
+    lib().sap_oracle_merge(o_a.ctypes.data_as(ctypes.c_void_p), lse_a.ctypes.data_as(ctypes.c_void_p),
+                           o_b.ctypes.data_as(ctypes.c_void_p), lse_b.ctypes.data_as(ctypes.c_void_p),
+                           ctypes.c_int64(n), ctypes.c_int(d),
+                           o.ctypes.data_as(ctypes.c_void_p), lse.ctypes.data_as(ctypes.c_void_p))
+    return o, lse
+
+
+def attn_bwd_dq(q, k, v, dout, cu_seqlens, scale: float, rows: Optional[Sequence[int]] = None):
+    q, qp = _f32(q); k, kp = _f32(k); v, vp = _f32(v); dout, dp = _f32(dout)
+    cu, cup = _i32(cu_seqlens)
+    N, Hq, Hkv, d = _dims(q, k)
+    rows_a, rp, nr = _i64_or_null(rows)
+    if rows is None:
+        nr = N
+    dq = np.empty((nr, Hq, d), dtype=np.float64)
+    rc = lib().sap_oracle_bwd_dq(qp, kp, vp, dp, cup, ctypes.c_int(len(cu) - 1), ctypes.c_int64(N),
+                                 ctypes.c_int(Hq), ctypes.c_int(Hkv), ctypes.c_int(d),
+                                 ctypes.c_double(scale), rp, ctypes.c_int64(nr),
+                                 dq.ctypes.data_as(ctypes.c_void_p))
+    if rc != 0:
+        raise ValueError("sap_oracle_bwd_dq: bad arguments")
+    return dq
+
+
+def attn_bwd_dkv(q, k, v, dout, cu_seqlens, scale: float, cols: Optional[Sequence[int]] = None):
+    q, qp = _f32(q); k, kp = _f32(k); v, vp = _f32(v); dout, dp = _f32(dout)
+    cu, cup = _i32(cu_seqlens)
+    N, Hq, Hkv, d = _dims(q, k)
+    cols_a, cp, nc = _i64_or_null(cols)
+    if cols is None:
+        nc = N
+    dk = np.empty((nc, Hkv, d), dtype=np.float64)
+    dv = np.empty((nc, Hkv, d), dtype=np.float64)
+    rc = lib().sap_oracle_bwd_dkv(qp, kp, vp, dp, cup, ctypes.c_int(len(cu) - 1), ctypes.c_int64(N),
+                                  ctypes.c_int(Hq), ctypes.c_int(Hkv), ctypes.c_int(d),
+                                  ctypes.c_double(scale), cp, ctypes.c_int64(nc),
+                                  dk.ctypes.data_as(ctypes.c_void_p), dv.ctypes.data_as(ctypes.c_void_p))
+    if rc != 0:
+        raise ValueError("sap_oracle_bwd_dkv: bad arguments")
+    return dk, dv
+
+
+class Plan:
+    """Result of the brute-definition planner."""
+
+    def __init__(self, items, chunk_offsets, kv_offsets, kv_index, kind_map):
+        self.items = items                  # int32 [n_items, 10]
+        self.chunk_offsets = chunk_offsets  # int32 [P+1]
+        self.kv_offsets = kv_offsets        # int32 [P+1]
+        self.kv_index = kv_index            # int32 [n_items]
+        self.kind_map = kind_map            # uint8 [P, P]
+
+    @property
+    def n_items(self):
+        return self.items.shape[0]
+
+
+def plan(cu_seqlens, n_chunks: int) -> Plan:
+    cu, cup = _i32(cu_seqlens)
+    P = int(n_chunks)
+    cap = max(1, P * (P + 1) // 2)
+    items = np.zeros((cap, 10), dtype=np.int32)
+    co = np.zeros(P + 1, dtype=np.int32)
+    ko = np.zeros(P + 1, dtype=np.int32)
+    ki = np.zeros(cap, dtype=np.int32)
+    km = np.zeros((P, P), dtype=np.uint8) if P > 0 else np.zeros((0, 0), dtype=np.uint8)
+    n = lib().sap_oracle_plan(cup, ctypes.c_int(len(cu) - 1), ctypes.c_int(P),
+                              items.ctypes.data_as(ctypes.c_void_p), co.ctypes.data_as(ctypes.c_void_p),
+                              ko.ctypes.data_as(ctypes.c_void_p), ki.ctypes.data_as(ctypes.c_void_p),
+                              km.ctypes.data_as(ctypes.c_void_p))
+    if n < 0:
+        raise ValueError({-1: "invalid argument", -2: "bad cu_seqlens", -3: "N not divisible by n_chunks"}[n])
+    return Plan(items[:n].copy(), co, ko, ki[:n].copy(), km)
