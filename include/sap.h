@@ -1,0 +1,149 @@
+/* sap.h — C ABI of the B200-native SAP attention hot path.
+ *
+ * Exact causal attention over a packed ("hybrid-context") sequence with no cross-document
+ * contamination, computed as partial attention between P sequence chunks (the paper's per-rank Q
+ * shards against incoming K/V shards, emulated on one GPU as chunks in HBM) and merged exactly
+ * through log-sum-exp.
+ *
+ * Citations are to /root/reference/PAPER.md (HSAP, arxiv/paper_2606_30460):
+ *   attention definition          §2.2.1, eq. at PAPER.md:55  Softmax(QK^T/sqrt(d))V, Q,K,V in R^{N x H x d} (:53)
+ *   packing / cu_len masking      §2.1, PAPER.md:39-45        "only compute attention within each segment", causal
+ *   chunks + online merge         §2.2.1, PAPER.md:59         blocks Q_i,K_i,V_i of n = N/P rows, merged "in an online manner"
+ *   JIT compile -> code lists     §3.1-3.2, Table 1 (:85-98): the `computing` instruction
+ *   "copy and rescale" fused      §6, PAPER.md:239 (the paper's stated future work; done in the kernel epilogue here)
+ *   backward tensors dq,dkv,do    Table 1
+ *
+ * Conventions
+ *   - Every function returns an int status (0 = SAP_OK); nothing throws, nothing aborts.
+ *   - "host" / "device" is stated per pointer.  Device buffers are owned by the caller; the library
+ *     allocates device memory only for a plan's device mirror (sap_plan_upload) and frees it in
+ *     sap_plan_destroy.  No call synchronises the device except sap_plan_upload.
+ *   - Layouts (packed "thd"): q/out/dout/dq  [N, Hq,  d] bf16, contiguous;
+ *     k/v/dk/dv [N, Hkv, d] bf16, contiguous; lse [Hq, N] fp32 (natural log of the sum of
+ *     exp(scale * q.k) over the visible keys); cu_seqlens int32 [D+1], cu[0] = 0, non-decreasing,
+ *     cu[D] = N.  q-head h reads kv-head h / (Hq/Hkv).
+ *   - Visibility: key s is visible to row t iff both lie in the same document and s <= t.
+ *   - head_dim in {64, 128}; Hq % Hkv == 0; N % n_chunks == 0 (contiguous equal chunks).
+ *   - All device pointers must be 16-byte aligned.
+ */
+#ifndef SAP_H_
+#define SAP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- status codes ------------------------------------------------------------------------- */
+enum {
+  SAP_OK = 0,
+  SAP_ERR_INVALID_ARG = 1,        /* null pointer, n_chunks < 1, n_docs < 1, bad range               */
+  SAP_ERR_BAD_CU_SEQLENS = 2,     /* cu[0] != 0, decreasing, or total length 0                        */
+  SAP_ERR_INDIVISIBLE = 3,        /* N % n_chunks != 0                                                */
+  SAP_ERR_UNSUPPORTED = 4,        /* head_dim not in {64,128}, Hq % Hkv != 0, misaligned pointer      */
+  SAP_ERR_WORKSPACE_TOO_SMALL = 5,
+  SAP_ERR_WRONG_ARCH = 6,         /* current device is not compute capability 10.x                    */
+  SAP_ERR_CUDA = 7,               /* a CUDA runtime/driver call failed; see sap_last_cuda_error()     */
+  SAP_ERR_NO_DEVICE = 8           /* no CUDA device / driver available                                */
+};
+
+/* ---- plan (host-side JIT planner; §3.2 Step 1, :106-:108) ------------------------- */
+enum { SAP_MASK_SKIP = 0, SAP_MASK_FULL = 1, SAP_MASK_DIAG = 2 };
+
+/* One `computing` work item (Table 1): partial attention of q-chunk i against
+ * kv-chunk j.  10 x int32, no padding, memcmp-comparable. */
+typedef struct {
+  int32_t q_chunk, kv_chunk;     /* i, j (j <= i)                                                   */
+  int32_t doc_lo, doc_hi;        /* inclusive range of contributing documents                        */
+  int32_t mask_kind;             /* SAP_MASK_FULL (no element masked inside the item's rectangle)    */
+                                 /* or SAP_MASK_DIAG (j == i: block-diagonal causal)                 */
+  int32_t step;                  /* ring step i - j                                                  */
+  int32_t q_begin, q_end;        /* absolute token range of rows that have visible keys, half-open   */
+  int32_t kv_begin, kv_end;      /* absolute token range of keys that are visible to some row        */
+} sap_item_t;
+
+typedef struct sap_plan sap_plan_t; /* opaque; immutable after creation except for the lazy device mirror */
+
+/* Build the plan for `cu_seqlens_host` (host, int32[n_docs+1]) split into `n_chunks` equal chunks.
+ * Keeps only chunk pairs whose documents intersect under causality, in ring order per q-chunk
+ * (step 0 = diagonal, then j = i-1, i-2, ...), and compiles the per-tile work lists the kernels
+ * walk.  Pure host code: works without a GPU.  *out is set only on SAP_OK. */
+int sap_plan_create(const int32_t* cu_seqlens_host, int32_t n_docs, int32_t n_chunks, sap_plan_t** out);
+void sap_plan_destroy(sap_plan_t* plan); /* frees host memory and the device mirror; NULL is a no-op */
+
+int32_t sap_plan_n_items(const sap_plan_t* plan);               /* number of non-SKIP items          */
+int32_t sap_plan_n_chunks(const sap_plan_t* plan);
+int32_t sap_plan_n_tokens(const sap_plan_t* plan);
+const sap_item_t* sap_plan_items(const sap_plan_t* plan);       /* host, plan-owned, [n_items]       */
+const int32_t* sap_plan_chunk_offsets(const sap_plan_t* plan);  /* host, [P+1], CSR by q_chunk       */
+const int32_t* sap_plan_kv_offsets(const sap_plan_t* plan);     /* host, [P+1], CSR by kv_chunk      */
+const int32_t* sap_plan_kv_index(const sap_plan_t* plan);       /* host, [n_items], item ids by kv_chunk */
+const uint8_t* sap_plan_kind_map(const sap_plan_t* plan);       /* host, [P*P] row-major, SKIP above diag */
+int64_t sap_plan_useful_pairs(const sap_plan_t* plan);          /* sum over documents of L(L+1)/2    */
+/* Number of 128x128 score tiles the forward kernel issues per q-head (for issue-efficiency reports). */
+int64_t sap_plan_fwd_tiles(const sap_plan_t* plan);
+
+/* Copy the compiled work lists to the current CUDA device (cudaMalloc + synchronous cudaMemcpy).
+ * Called implicitly by the first sap_attn_* call that uses the plan; call it yourself to keep that
+ * cost out of a timed region.  Idempotent, thread-safe. */
+int sap_plan_upload(sap_plan_t* plan);
+
+/* ---- attention ------------------------------------------------------------------------------ */
+enum { SAP_PASS_FWD = 0, SAP_PASS_BWD = 1 };
+
+/* Bytes of caller-provided device workspace a pass needs (fwd: 0; bwd: D = rowsum(dO*O), fp32 [Hq,N]). */
+size_t sap_workspace_bytes(const sap_plan_t* plan, int n_q_heads, int n_kv_heads, int head_dim, int pass);
+
+/* Forward: for every row, attention over the visible keys, walking the row's
+ * q-chunk items in plan order and merging the per-item partials on chip (running max / sum / O).
+ * q,k,v,cu_seqlens_dev: device, read.  out: device bf16 [N,Hq,d], written.  lse: device fp32 [Hq,N], written.
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Asynchronous. */
+int sap_attn_fwd(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev,
+                 sap_plan_t* plan, void* out, float* lse,
+                 int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
+                 void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Partial forward over plan items [item_begin, item_end) only (ids index sap_plan_items).
+ * out_f32: device fp32 [N,Hq,d], normalised partial output; lse: device fp32 [Hq,N].
+ * Rows with no visible key among those items get out = 0, lse = -inf.  Items of one q-chunk cover
+ * disjoint key sets, so partials of disjoint item sets merge exactly with sap_lse_merge. */
+int sap_attn_fwd_partial(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev,
+                         sap_plan_t* plan, int32_t item_begin, int32_t item_end,
+                         float* out_f32, float* lse,
+                         int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
+                         void* cuda_stream);
+
+/* Exact merge of two partials over disjoint key sets (online softmax; "rescale", :239):
+ *   L = max(La,Lb) + ln(e^{La-max} + e^{Lb-max});  O = e^{La-L} Oa + e^{Lb-L} Ob;  (-inf, 0) is the identity.
+ * o_a,o_b: device fp32 [N,Hq,d]; lse_a,lse_b: device fp32 [Hq,N]; o_out: device, fp32 or bf16
+ * (out_is_bf16 != 0) [N,Hq,d]; lse_out: device fp32 [Hq,N].  Outputs may alias the `a` inputs.
+ * Only rows [row_begin,row_end) are read and written. */
+int sap_lse_merge(const float* o_a, const float* lse_a, const float* o_b, const float* lse_b,
+                  void* o_out, int out_is_bf16, float* lse_out,
+                  int64_t n_tokens, int n_q_heads, int head_dim, int64_t row_begin, int64_t row_end,
+                  void* cuda_stream);
+
+/* Backward (Table 1 tensors do/dq/dkv).  With P = exp(scale*QK^T - LSE) on the visible
+ * pairs: D_t = sum_c dO_tc O_tc; dP = dO V^T; dS = P*(dP - D); dQ = scale dS K; dK = scale dS^T Q;
+ * dV = P^T dO; dK/dV are summed over the Hq/Hkv q-heads of a group.
+ * dout,q,k,v,out,lse,cu_seqlens_dev: device, read (out/lse as written by sap_attn_fwd).
+ * dq [N,Hq,d], dk,dv [N,Hkv,d]: device bf16, written (every element).  workspace: device, at least
+ * sap_workspace_bytes(plan, ..., SAP_PASS_BWD) bytes. */
+int sap_attn_bwd(const void* dout, const void* q, const void* k, const void* v, const void* out,
+                 const float* lse, const int32_t* cu_seqlens_dev, sap_plan_t* plan,
+                 void* dq, void* dk, void* dv,
+                 int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
+                 void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---- diagnostics ---------------------------------------------------------------------------- */
+const char* sap_strerror(int status);
+int sap_last_cuda_error(void);      /* the cudaError_t / CUresult of the last SAP_ERR_CUDA on this thread */
+/* Number of kernels the library has launched in this process (all streams); for launch accounting. */
+int64_t sap_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SAP_H_ */

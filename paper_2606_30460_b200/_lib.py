@@ -1,0 +1,65 @@
+"""Loads libsap_b200.so and declares the C ABI of include/sap.h for ctypes.  No fallback: a missing
+library is an ImportError-class failure (RuntimeError), never a silent CPU path."""
+from __future__ import annotations
+
+import ctypes
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libsap_b200.so")
+
+c_i32p = ctypes.POINTER(ctypes.c_int32)
+c_f32p = ctypes.POINTER(ctypes.c_float)
+vp = ctypes.c_void_p
+
+
+class SapItem(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("q_chunk", "kv_chunk", "doc_lo", "doc_hi", "mask_kind", "step",
+                                             "q_begin", "q_end", "kv_begin", "kv_end")]
+
+
+# name -> (restype, argtypes); mirrors include/sap.h one to one
+SIGNATURES = {
+    "sap_plan_create": (ctypes.c_int, [vp, ctypes.c_int32, ctypes.c_int32, ctypes.POINTER(vp)]),
+    "sap_plan_destroy": (None, [vp]),
+    "sap_plan_n_items": (ctypes.c_int32, [vp]),
+    "sap_plan_n_chunks": (ctypes.c_int32, [vp]),
+    "sap_plan_n_tokens": (ctypes.c_int32, [vp]),
+    "sap_plan_items": (ctypes.POINTER(SapItem), [vp]),
+    "sap_plan_chunk_offsets": (c_i32p, [vp]),
+    "sap_plan_kv_offsets": (c_i32p, [vp]),
+    "sap_plan_kv_index": (c_i32p, [vp]),
+    "sap_plan_kind_map": (ctypes.POINTER(ctypes.c_uint8), [vp]),
+    "sap_plan_useful_pairs": (ctypes.c_int64, [vp]),
+    "sap_plan_fwd_tiles": (ctypes.c_int64, [vp]),
+    "sap_plan_upload": (ctypes.c_int, [vp]),
+    "sap_workspace_bytes": (ctypes.c_size_t, [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
+    "sap_attn_fwd": (ctypes.c_int, [vp, vp, vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                    ctypes.c_float, vp, ctypes.c_size_t, vp]),
+    "sap_attn_fwd_partial": (ctypes.c_int, [vp, vp, vp, vp, vp, ctypes.c_int32, ctypes.c_int32, vp, vp,
+                                            ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_float, vp]),
+    "sap_lse_merge": (ctypes.c_int, [vp, vp, vp, vp, vp, ctypes.c_int, vp, ctypes.c_int64, ctypes.c_int,
+                                     ctypes.c_int, ctypes.c_int64, ctypes.c_int64, vp]),
+    "sap_attn_bwd": (ctypes.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int,
+                                    ctypes.c_int, ctypes.c_float, vp, ctypes.c_size_t, vp]),
+    "sap_strerror": (ctypes.c_char_p, [ctypes.c_int]),
+    "sap_last_cuda_error": (ctypes.c_int, []),
+    "sap_launch_count": (ctypes.c_int64, []),
+}
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_30460_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)          # AttributeError if the symbol is not exported
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib

@@ -1,0 +1,199 @@
+"""Thin Python binding of include/sap.h: argument marshalling only (torch is used for device memory
+and streams); every step of the hot path runs in the CUDA kernels behind the C ABI."""
+from __future__ import annotations
+
+import ctypes
+from typing import Optional, Sequence
+
+import numpy as np
+
+from . import _lib
+
+SAP_MASK_SKIP, SAP_MASK_FULL, SAP_MASK_DIAG = 0, 1, 2
+SAP_PASS_FWD, SAP_PASS_BWD = 0, 1
+
+
+class SapError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        L = _lib.lib()
+        msg = L.sap_strerror(status).decode()
+        extra = f" (cuda error {L.sap_last_cuda_error()})" if status == 7 else ""
+        super().__init__(f"{where}: {msg}{extra}")
+        self.status = status
+
+
+def _check(status: int, where: str):
+    if status != 0:
+        raise SapError(status, where)
+
+
+def _ptr(t) -> ctypes.c_void_p:
+    return ctypes.c_void_p(0 if t is None else t.data_ptr())
+
+
+def _stream(stream) -> ctypes.c_void_p:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+class Plan:
+    """sap_plan: host-side JIT planner result (items in ring order + compiled tile programs)."""
+
+    def __init__(self, cu_seqlens: Sequence[int], n_chunks: int):
+        cu = np.ascontiguousarray(np.asarray(cu_seqlens, dtype=np.int64).astype(np.int32))
+        self._cu_host = cu
+        self._h = ctypes.c_void_p(0)
+        self._cu_dev = {}
+        L = _lib.lib()
+        _check(L.sap_plan_create(cu.ctypes.data_as(ctypes.c_void_p), len(cu) - 1, int(n_chunks),
+                                 ctypes.byref(self._h)), "sap_plan_create")
+        self.n_chunks = int(n_chunks)
+        self.n_tokens = int(L.sap_plan_n_tokens(self._h))
+        self.n_items = int(L.sap_plan_n_items(self._h))
+
+    def __del__(self):
+        h = getattr(self, "_h", None)
+        if h is not None and h.value:
+            _lib.lib().sap_plan_destroy(h)
+            self._h = ctypes.c_void_p(0)
+
+    @property
+    def handle(self) -> ctypes.c_void_p:
+        return self._h
+
+    @property
+    def items(self) -> np.ndarray:
+        """int32 [n_items, 10] in sap_item_t field order."""
+        p = _lib.lib().sap_plan_items(self._h)
+        n = self.n_items
+        if n == 0:
+            return np.zeros((0, 10), dtype=np.int32)
+        return np.ctypeslib.as_array(ctypes.cast(p, _lib.c_i32p), shape=(n, 10)).copy()
+
+    def _arr(self, fn, n):
+        return np.ctypeslib.as_array(fn(self._h), shape=(n,)).copy()
+
+    @property
+    def chunk_offsets(self) -> np.ndarray:
+        return self._arr(_lib.lib().sap_plan_chunk_offsets, self.n_chunks + 1)
+
+    @property
+    def kv_offsets(self) -> np.ndarray:
+        return self._arr(_lib.lib().sap_plan_kv_offsets, self.n_chunks + 1)
+
+    @property
+    def kv_index(self) -> np.ndarray:
+        return self._arr(_lib.lib().sap_plan_kv_index, self.n_items) if self.n_items else np.zeros(0, np.int32)
+
+    @property
+    def kind_map(self) -> np.ndarray:
+        P = self.n_chunks
+        return self._arr(_lib.lib().sap_plan_kind_map, P * P).reshape(P, P)
+
+    @property
+    def useful_pairs(self) -> int:
+        return int(_lib.lib().sap_plan_useful_pairs(self._h))
+
+    @property
+    def fwd_tiles(self) -> int:
+        return int(_lib.lib().sap_plan_fwd_tiles(self._h))
+
+    def upload(self):
+        _check(_lib.lib().sap_plan_upload(self._h), "sap_plan_upload")
+
+    def cu_seqlens_dev(self, device):
+        import torch
+        key = str(device)
+        if key not in self._cu_dev:
+            self._cu_dev[key] = torch.from_numpy(self._cu_host).to(device)
+        return self._cu_dev[key]
+
+
+def sap_plan(cu_seqlens: Sequence[int], n_chunks: int) -> Plan:
+    return Plan(cu_seqlens, n_chunks)
+
+
+def sap_workspace_bytes(plan: Plan, n_q_heads: int, n_kv_heads: int, head_dim: int, pass_: int) -> int:
+    return int(_lib.lib().sap_workspace_bytes(plan.handle, n_q_heads, n_kv_heads, head_dim, pass_))
+
+
+def _dims(q, k):
+    N, Hq, d = q.shape
+    return int(N), int(Hq), int(k.shape[1]), int(d)
+
+
+def _require_cuda_bf16(*ts):
+    import torch
+    for t in ts:
+        if not (t.is_cuda and t.dtype == torch.bfloat16 and t.is_contiguous()):
+            raise ValueError("expected contiguous CUDA bf16 tensors")
+
+
+def sap_attn_fwd(q, k, v, cu_seqlens_dev, plan: Plan, out=None, lse=None, softmax_scale: Optional[float] = None,
+                 stream=None):
+    """out [N,Hq,d] bf16, lse [Hq,N] fp32 = sap_attn_fwd(...).  Asynchronous on `stream`."""
+    import torch
+    _require_cuda_bf16(q, k, v)
+    N, Hq, Hkv, d = _dims(q, k)
+    if out is None:
+        out = torch.empty_like(q)
+    if lse is None:
+        lse = torch.empty((Hq, N), dtype=torch.float32, device=q.device)
+    scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
+    _check(_lib.lib().sap_attn_fwd(_ptr(q), _ptr(k), _ptr(v), _ptr(cu_seqlens_dev), plan.handle, _ptr(out),
+                                   _ptr(lse), Hq, Hkv, d, scale, None, 0, _stream(stream)), "sap_attn_fwd")
+    return out, lse
+
+
+def sap_attn_fwd_partial(q, k, v, cu_seqlens_dev, plan: Plan, item_begin: int, item_end: int,
+                         softmax_scale: Optional[float] = None, stream=None):
+    """Partial forward over plan items [item_begin, item_end): (out fp32 [N,Hq,d], lse fp32 [Hq,N])."""
+    import torch
+    _require_cuda_bf16(q, k, v)
+    N, Hq, Hkv, d = _dims(q, k)
+    out = torch.empty((N, Hq, d), dtype=torch.float32, device=q.device)
+    lse = torch.empty((Hq, N), dtype=torch.float32, device=q.device)
+    scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
+    _check(_lib.lib().sap_attn_fwd_partial(_ptr(q), _ptr(k), _ptr(v), _ptr(cu_seqlens_dev), plan.handle,
+                                           int(item_begin), int(item_end), _ptr(out), _ptr(lse), Hq, Hkv, d, scale,
+                                           _stream(stream)), "sap_attn_fwd_partial")
+    return out, lse
+
+
+def sap_lse_merge(o_a, lse_a, o_b, lse_b, out_bf16: bool = False, row_begin: int = 0,
+                  row_end: Optional[int] = None, o_out=None, lse_out=None, stream=None):
+    import torch
+    N, Hq, d = o_a.shape
+    row_end = N if row_end is None else row_end
+    if o_out is None:
+        o_out = torch.zeros((N, Hq, d), dtype=torch.bfloat16 if out_bf16 else torch.float32, device=o_a.device)
+    if lse_out is None:
+        lse_out = torch.full((Hq, N), float("-inf"), dtype=torch.float32, device=o_a.device)
+    _check(_lib.lib().sap_lse_merge(_ptr(o_a), _ptr(lse_a), _ptr(o_b), _ptr(lse_b), _ptr(o_out), int(out_bf16),
+                                    _ptr(lse_out), N, Hq, d, int(row_begin), int(row_end), _stream(stream)),
+           "sap_lse_merge")
+    return o_out, lse_out
+
+
+def sap_attn_bwd(dout, q, k, v, out, lse, cu_seqlens_dev, plan: Plan, softmax_scale: Optional[float] = None,
+                 dq=None, dk=None, dv=None, workspace=None, stream=None):
+    """dq [N,Hq,d], dk, dv [N,Hkv,d] bf16 = sap_attn_bwd(...).  Asynchronous on `stream`."""
+    import torch
+    _require_cuda_bf16(dout, q, k, v, out)
+    N, Hq, Hkv, d = _dims(q, k)
+    dq = torch.empty_like(q) if dq is None else dq
+    dk = torch.empty_like(k) if dk is None else dk
+    dv = torch.empty_like(v) if dv is None else dv
+    need = sap_workspace_bytes(plan, Hq, Hkv, d, SAP_PASS_BWD)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=q.device)
+    scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
+    _check(_lib.lib().sap_attn_bwd(_ptr(dout), _ptr(q), _ptr(k), _ptr(v), _ptr(out), _ptr(lse),
+                                   _ptr(cu_seqlens_dev), plan.handle, _ptr(dq), _ptr(dk), _ptr(dv), Hq, Hkv, d,
+                                   scale, _ptr(workspace), workspace.numel(), _stream(stream)), "sap_attn_bwd")
+    return dq, dk, dv
+
+
+def sap_launch_count() -> int:
+    return int(_lib.lib().sap_launch_count())

@@ -1,0 +1,228 @@
+// C-ABI entry points that touch the GPU (include/sap.h): plan upload, forward, partial forward,
+// LSE merge, backward.  Argument checking + tensor-map encoding + launches only.
+#include <cstdio>
+#include <cstring>
+#include "sap_host.h"
+#include "sap_fwd.cuh"
+#include "sap_bwd.cuh"
+#include "sap_merge.cuh"
+
+namespace sap {
+
+thread_local int g_last_cuda_error = 0;
+std::atomic<int64_t> g_launch_count{0};
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = []() -> EncodeTiledFn {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess) return nullptr;
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+int make_tile_map(CUtensorMap* map, const void* base, int64_t n_rows, int64_t row_elems) {
+  EncodeTiledFn enc = get_encode_fn();
+  if (!enc) { g_last_cuda_error = static_cast<int>(cudaErrorNotSupported); return SAP_ERR_CUDA; }
+  cuuint64_t dims[2] = {static_cast<cuuint64_t>(row_elems), static_cast<cuuint64_t>(n_rows)};
+  cuuint64_t strides[1] = {static_cast<cuuint64_t>(row_elems) * 2};
+  cuuint32_t box[2] = {64, static_cast<cuuint32_t>(kTile)};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { g_last_cuda_error = static_cast<int>(r); return SAP_ERR_CUDA; }
+  return SAP_OK;
+}
+
+int check_device_is_sm100() {
+  int dev = 0;
+  SAP_CUDA_CHECK(cudaGetDevice(&dev));
+  static int cached_dev = -1, cached_major = 0;
+  if (cached_dev != dev) {
+    int major = 0;
+    SAP_CUDA_CHECK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    cached_major = major; cached_dev = dev;
+  }
+  return cached_major == 10 ? SAP_OK : SAP_ERR_WRONG_ARCH;
+}
+
+int upload_program(const TileProgram& host, DevProgram& dev) {
+  dev.n_tiles = static_cast<int32_t>(host.tiles.size());
+  const size_t tb = host.tiles.size() * sizeof(TileDesc), sb = (host.segs.size() + 1) * sizeof(SegDesc);
+  SAP_CUDA_CHECK(cudaMalloc(&dev.tiles, tb ? tb : sizeof(TileDesc)));
+  SAP_CUDA_CHECK(cudaMalloc(&dev.segs, sb));
+  if (tb) SAP_CUDA_CHECK(cudaMemcpy(dev.tiles, host.tiles.data(), tb, cudaMemcpyHostToDevice));
+  if (!host.segs.empty())
+    SAP_CUDA_CHECK(cudaMemcpy(dev.segs, host.segs.data(), host.segs.size() * sizeof(SegDesc), cudaMemcpyHostToDevice));
+  return SAP_OK;
+}
+
+void free_program(DevProgram& dev) {
+  if (dev.tiles) cudaFree(dev.tiles);
+  if (dev.segs) cudaFree(dev.segs);
+  dev = DevProgram();
+}
+
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static int check_dims(const sap_plan_t* plan, int Hq, int Hkv, int d, float scale) {
+  if (!plan) return SAP_ERR_INVALID_ARG;
+  if (Hq < 1 || Hkv < 1 || !(scale > 0.f)) return SAP_ERR_INVALID_ARG;
+  if ((d != 64 && d != 128) || Hq % Hkv != 0) return SAP_ERR_UNSUPPORTED;
+  return SAP_OK;
+}
+
+template <int D, bool PARTIAL>
+static int launch_fwd(const DevProgram& prog, const void* q, const void* k, const void* v, const int32_t* cu,
+                      const sap_plan_t* plan, void* out, float* out_f32, float* lse, int Hq, int Hkv, float scale,
+                      cudaStream_t stream) {
+  CUtensorMap mq, mk, mv;
+  int rc;
+  if ((rc = make_tile_map(&mq, q, plan->n_tokens, (int64_t)Hq * D)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mk, k, plan->n_tokens, (int64_t)Hkv * D)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mv, v, plan->n_tokens, (int64_t)Hkv * D)) != SAP_OK) return rc;
+  auto kern = sap_fwd_kernel<D, PARTIAL>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    SAP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdSmem<D>::kTotal));
+    attr_set = true;
+  }
+  const unsigned grid = static_cast<unsigned>(prog.n_tiles) * Hq;
+  kern<<<grid, kFwdThreads, FwdSmem<D>::kTotal, stream>>>(mq, mk, mv, prog.tiles, prog.segs, cu, plan->n_docs,
+                                                          static_cast<__nv_bfloat16*>(out), out_f32, lse,
+                                                          plan->n_tokens, Hq, Hkv, scale * kLog2e);
+  g_launch_count.fetch_add(1);
+  SAP_CUDA_CHECK(cudaGetLastError());
+  return SAP_OK;
+}
+
+}  // namespace sap
+
+using namespace sap;
+
+extern "C" {
+
+int sap_last_cuda_error(void) { return g_last_cuda_error; }
+int64_t sap_launch_count(void) { return g_launch_count.load(); }
+
+int sap_plan_upload(sap_plan_t* plan) {
+  if (!plan) return SAP_ERR_INVALID_ARG;
+  std::lock_guard<std::mutex> lock(plan->mu);
+  PlanDevice* pd = static_cast<PlanDevice*>(plan->dev_state);
+  if (pd && pd->uploaded) return SAP_OK;
+  int rc = check_device_is_sm100();
+  if (rc != SAP_OK) return rc;
+  if (!pd) { pd = new PlanDevice(); plan->dev_state = pd; }
+  SAP_CUDA_CHECK(cudaGetDevice(&pd->device));
+  if ((rc = upload_program(plan->fwd, pd->fwd)) != SAP_OK) return rc;
+  if ((rc = upload_program(plan->kv, pd->kv)) != SAP_OK) return rc;
+  pd->uploaded = true;
+  return SAP_OK;
+}
+
+void sap_plan_destroy(sap_plan_t* plan) {
+  if (!plan) return;
+  PlanDevice* pd = static_cast<PlanDevice*>(plan->dev_state);
+  if (pd) {
+    free_program(pd->fwd);
+    free_program(pd->kv);
+    for (auto& kv : pd->partial) free_program(kv.second);
+    delete pd;
+  }
+  delete plan;
+}
+
+size_t sap_workspace_bytes(const sap_plan_t* plan, int n_q_heads, int n_kv_heads, int head_dim, int pass) {
+  (void)n_kv_heads; (void)head_dim;
+  if (!plan || pass != SAP_PASS_BWD) return 0;
+  return static_cast<size_t>(plan->n_tokens) * n_q_heads * sizeof(float);  // D = rowsum(dO * O), fp32 [Hq, N]
+}
+
+int sap_attn_fwd(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev, sap_plan_t* plan,
+                 void* out, float* lse, int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
+                 void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  (void)workspace; (void)workspace_bytes;
+  if (!q || !k || !v || !cu_seqlens_dev || !out || !lse) return SAP_ERR_INVALID_ARG;
+  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  if (rc != SAP_OK) return rc;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out)) return SAP_ERR_UNSUPPORTED;
+  if ((rc = sap_plan_upload(plan)) != SAP_OK) return rc;
+  const PlanDevice* pd = static_cast<const PlanDevice*>(plan->dev_state);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (head_dim == 128)
+    return launch_fwd<128, false>(pd->fwd, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st);
+  return launch_fwd<64, false>(pd->fwd, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st);
+}
+
+int sap_attn_fwd_partial(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev, sap_plan_t* plan,
+                         int32_t item_begin, int32_t item_end, float* out_f32, float* lse, int n_q_heads,
+                         int n_kv_heads, int head_dim, float softmax_scale, void* cuda_stream) {
+  if (!q || !k || !v || !cu_seqlens_dev || !out_f32 || !lse) return SAP_ERR_INVALID_ARG;
+  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  if (rc != SAP_OK) return rc;
+  if (item_begin < 0 || item_end < item_begin || item_end > (int32_t)plan->items.size()) return SAP_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out_f32)) return SAP_ERR_UNSUPPORTED;
+  if ((rc = sap_plan_upload(plan)) != SAP_OK) return rc;
+  PlanDevice* pd = static_cast<PlanDevice*>(plan->dev_state);
+  DevProgram prog;
+  {
+    std::lock_guard<std::mutex> lock(plan->mu);
+    auto key = std::make_pair(item_begin, item_end);
+    auto itp = pd->partial.find(key);
+    if (itp == pd->partial.end()) {
+      TileProgram host;
+      build_q_program(*plan, item_begin, item_end, host);
+      DevProgram dp;
+      if ((rc = upload_program(host, dp)) != SAP_OK) return rc;
+      itp = pd->partial.emplace(key, dp).first;
+    }
+    prog = itp->second;
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (head_dim == 128)
+    return launch_fwd<128, true>(prog, q, k, v, cu_seqlens_dev, plan, nullptr, out_f32, lse, n_q_heads, n_kv_heads, softmax_scale, st);
+  return launch_fwd<64, true>(prog, q, k, v, cu_seqlens_dev, plan, nullptr, out_f32, lse, n_q_heads, n_kv_heads, softmax_scale, st);
+}
+
+int sap_lse_merge(const float* o_a, const float* lse_a, const float* o_b, const float* lse_b, void* o_out,
+                  int out_is_bf16, float* lse_out, int64_t n_tokens, int n_q_heads, int head_dim, int64_t row_begin,
+                  int64_t row_end, void* cuda_stream) {
+  if (!o_a || !lse_a || !o_b || !lse_b || !o_out || !lse_out) return SAP_ERR_INVALID_ARG;
+  if (n_tokens < 1 || n_q_heads < 1 || row_begin < 0 || row_end < row_begin || row_end > n_tokens) return SAP_ERR_INVALID_ARG;
+  if (head_dim < 4 || head_dim % 4 != 0) return SAP_ERR_UNSUPPORTED;
+  if (!aligned16(o_a) || !aligned16(o_b) || (reinterpret_cast<uintptr_t>(o_out) & 7u)) return SAP_ERR_UNSUPPORTED;
+  int rc = check_device_is_sm100();
+  if (rc != SAP_OK) return rc;
+  const int64_t n_rows = (row_end - row_begin) * n_q_heads;
+  if (n_rows == 0) return SAP_OK;
+  const int vec = head_dim / 4;
+  const int group = (vec <= 32 && (vec & (vec - 1)) == 0) ? vec : 32;
+  const int64_t want = (n_rows * group + kMergeThreads - 1) / kMergeThreads;
+  const unsigned grid = static_cast<unsigned>(want < 148 * 16 ? want : 148 * 16);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (out_is_bf16)
+    sap_lse_merge_kernel<true><<<grid, kMergeThreads, 0, st>>>(o_a, lse_a, o_b, lse_b, o_out, lse_out, n_tokens, n_q_heads, head_dim, row_begin, n_rows, group);
+  else
+    sap_lse_merge_kernel<false><<<grid, kMergeThreads, 0, st>>>(o_a, lse_a, o_b, lse_b, o_out, lse_out, n_tokens, n_q_heads, head_dim, row_begin, n_rows, group);
+  g_launch_count.fetch_add(1);
+  SAP_CUDA_CHECK(cudaGetLastError());
+  return SAP_OK;
+}
+
+int sap_attn_bwd(const void* dout, const void* q, const void* k, const void* v, const void* out, const float* lse,
+                 const int32_t* cu_seqlens_dev, sap_plan_t* plan, void* dq, void* dk, void* dv, int n_q_heads,
+                 int n_kv_heads, int head_dim, float softmax_scale, void* workspace, size_t workspace_bytes,
+                 void* cuda_stream) {
+  (void)dout; (void)q; (void)k; (void)v; (void)out; (void)lse; (void)cu_seqlens_dev; (void)plan; (void)dq; (void)dk;
+  (void)dv; (void)n_q_heads; (void)n_kv_heads; (void)head_dim; (void)softmax_scale; (void)workspace;
+  (void)workspace_bytes; (void)cuda_stream;
+  return SAP_ERR_UNSUPPORTED;
+}
+
+}  // extern "C"

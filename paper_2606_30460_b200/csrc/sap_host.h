@@ -1,0 +1,46 @@
+// Host-side helpers of the CUDA half of the library: error bookkeeping, tensor-map encoding,
+// device mirrors of the tile programs.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <atomic>
+#include <map>
+#include <utility>
+#include "sap_internal.h"
+
+namespace sap {
+
+extern thread_local int g_last_cuda_error;
+extern std::atomic<int64_t> g_launch_count;
+
+#define SAP_CUDA_CHECK(expr)                                   \
+  do {                                                         \
+    cudaError_t _e = (expr);                                   \
+    if (_e != cudaSuccess) {                                   \
+      sap::g_last_cuda_error = static_cast<int>(_e);           \
+      return (_e == cudaErrorNoDevice || _e == cudaErrorInsufficientDriver) ? SAP_ERR_NO_DEVICE : SAP_ERR_CUDA; \
+    }                                                          \
+  } while (0)
+
+struct DevProgram {
+  TileDesc* tiles = nullptr;
+  SegDesc* segs = nullptr;
+  int32_t n_tiles = 0;
+};
+
+// Device copies owned by a plan (freed by sap_plan_destroy).
+struct PlanDevice {
+  bool uploaded = false;
+  int device = -1;
+  DevProgram fwd, kv;
+  std::map<std::pair<int32_t, int32_t>, DevProgram> partial;  // item-range-restricted Q programs
+};
+
+int check_device_is_sm100();
+int upload_program(const TileProgram& host, DevProgram& dev);
+void free_program(DevProgram& dev);
+
+// 2D bf16 tensor map over a [n_rows, n_heads*head_dim] matrix, box = 64 columns x 128 rows, 128-byte swizzle.
+int make_tile_map(CUtensorMap* map, const void* base, int64_t n_rows, int64_t row_elems);
+
+}  // namespace sap

@@ -1,0 +1,220 @@
+// Host-side JIT planner (§3.1-3.2: "compile" side of SAP's compile-execute split, :75,:106-:120).
+//
+// Step 1 of the paper's compiler partitions the attention mask by rank rows/columns and classifies
+// each (q_chunk, kv_chunk) block (:108).  With contiguous equal chunks (n = N/P, :59) and the cu_len
+// visibility rule (:45) the classification has a closed form, used here (the oracle's planner instead
+// loops over all documents for every pair):
+//   * j == i : DIAG.  Rows = keys = the whole chunk; documents doc(i*n) .. doc((i+1)*n - 1).
+//   * j <  i : at most one document can reach back into chunk j: e* = doc(i*n), and it does iff
+//              cu[e*] < (j+1)*n.  Rows [i*n, min(cu[e*+1], (i+1)*n)), keys [max(cu[e*], j*n), (j+1)*n);
+//              every (row, key) of that rectangle is visible => FULL needs no mask.
+// doc(t) = the unique e with cu[e] <= t < cu[e+1] (zero-length documents never contain a token).
+//
+// The planner then "jits" the item lists into per-tile programs (TileDesc/SegDesc) the kernels walk:
+// the analogue of the paper's per-rank instruction lists (:120), at 128-row tile granularity.
+#include <algorithm>
+#include <cstring>
+#include <new>
+#include "sap_internal.h"
+
+namespace sap {
+
+static inline int32_t doc_of(const std::vector<int32_t>& cu, int64_t t) {
+  // last e with cu[e] <= t  (upper_bound - 1); skips zero-length documents automatically
+  return (int32_t)(std::upper_bound(cu.begin(), cu.end(), (int32_t)t) - cu.begin()) - 1;
+}
+
+static inline int32_t floor_tile(int64_t x) { return (int32_t)(x / kTile * kTile); }
+
+void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, TileProgram& out) {
+  out.tiles.clear();
+  out.segs.clear();
+  out.streamed_tiles = 0;
+  const int64_t n = p.chunk_len;
+  std::vector<int64_t> work;
+  for (int32_t i = 0; i < p.n_chunks; ++i) {
+    const int64_t c_begin = (int64_t)i * n, c_end = c_begin + n;
+    for (int64_t r0 = c_begin; r0 < c_end; r0 += kTile) {
+      const int64_t r1 = std::min<int64_t>(r0 + kTile, c_end);
+      TileDesc td;
+      td.row0 = (int32_t)r0;
+      td.rows = (int32_t)(r1 - r0);
+      td.seg_begin = (int32_t)out.segs.size();
+      int64_t w = 0;
+      for (int32_t it = p.chunk_offsets[i]; it < p.chunk_offsets[i + 1]; ++it) {
+        if (it < item_begin || it >= item_end) continue;
+        const sap_item_t& im = p.items[it];
+        const int64_t ra = std::max<int64_t>(r0, im.q_begin), rb = std::min<int64_t>(r1, im.q_end);
+        if (ra >= rb) continue;
+        // keys needed by rows [ra, rb): from the start of the first row's document up to the last row
+        const int64_t lo = std::max<int64_t>(im.kv_begin, p.cu[doc_of(p.cu, ra)]);
+        const int64_t hi = std::min<int64_t>(im.kv_end, rb);
+        if (lo >= hi) continue;
+        SegDesc sd;
+        sd.t_begin = floor_tile(lo);
+        sd.t_end = (int32_t)hi;
+        sd.q_lo = im.q_begin; sd.q_hi = im.q_end;
+        sd.kv_lo = im.kv_begin; sd.kv_hi = im.kv_end;
+        sd.item = it; sd.pad = 0;
+        out.segs.push_back(sd);
+        w += (hi - sd.t_begin + kTile - 1) / kTile;
+      }
+      td.seg_end = (int32_t)out.segs.size();
+      out.tiles.push_back(td);
+      work.push_back(w);
+      out.streamed_tiles += w;
+    }
+  }
+  // longest first (LPT): the hardware block scheduler hands tiles out in blockIdx order
+  std::vector<int32_t> order(out.tiles.size());
+  for (size_t k = 0; k < order.size(); ++k) order[k] = (int32_t)k;
+  std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return work[a] > work[b]; });
+  std::vector<TileDesc> sorted(out.tiles.size());
+  for (size_t k = 0; k < order.size(); ++k) sorted[k] = out.tiles[order[k]];
+  out.tiles.swap(sorted);
+}
+
+void build_kv_program(const sap_plan& p, TileProgram& out) {
+  out.tiles.clear();
+  out.segs.clear();
+  out.streamed_tiles = 0;
+  const int64_t n = p.chunk_len, N = p.n_tokens;
+  std::vector<int64_t> work;
+  // K/V tiles are globally 128-aligned (they must match the key tiles the forward kernel streams only in
+  // coverage, not in alignment); a tile that straddles two kv-chunks gets segments from both.
+  for (int64_t c0 = 0; c0 < N; c0 += kTile) {
+    const int64_t c1 = std::min<int64_t>(c0 + kTile, N);
+    TileDesc td;
+    td.row0 = (int32_t)c0;
+    td.rows = (int32_t)(c1 - c0);
+    td.seg_begin = (int32_t)out.segs.size();
+    int64_t w = 0;
+    const int32_t j_lo = (int32_t)(c0 / n), j_hi = (int32_t)((c1 - 1) / n);
+    for (int32_t j = j_lo; j <= j_hi; ++j) {
+      for (int32_t x = p.kv_offsets[j]; x < p.kv_offsets[j + 1]; ++x) {
+        const int32_t it = p.kv_index[x];
+        const sap_item_t& im = p.items[it];
+        const int64_t ca = std::max<int64_t>(c0, im.kv_begin), cb = std::min<int64_t>(c1, im.kv_end);
+        if (ca >= cb) continue;
+        // rows that see keys [ca, cb): from the first key up to the end of the last key's document
+        const int64_t lo = std::max<int64_t>(im.q_begin, ca);
+        const int64_t hi = std::min<int64_t>(im.q_end, p.cu[doc_of(p.cu, cb - 1) + 1]);
+        if (lo >= hi) continue;
+        SegDesc sd;
+        sd.t_begin = floor_tile(lo);
+        sd.t_end = (int32_t)hi;
+        sd.q_lo = im.q_begin; sd.q_hi = im.q_end;
+        sd.kv_lo = im.kv_begin; sd.kv_hi = im.kv_end;
+        sd.item = it; sd.pad = 0;
+        out.segs.push_back(sd);
+        w += (hi - sd.t_begin + kTile - 1) / kTile;
+      }
+    }
+    td.seg_end = (int32_t)out.segs.size();
+    out.tiles.push_back(td);
+    work.push_back(w);
+    out.streamed_tiles += w;
+  }
+  std::vector<int32_t> order(out.tiles.size());
+  for (size_t k = 0; k < order.size(); ++k) order[k] = (int32_t)k;
+  std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return work[a] > work[b]; });
+  std::vector<TileDesc> sorted(out.tiles.size());
+  for (size_t k = 0; k < order.size(); ++k) sorted[k] = out.tiles[order[k]];
+  out.tiles.swap(sorted);
+}
+
+}  // namespace sap
+
+using namespace sap;
+
+extern "C" {
+
+int sap_plan_create(const int32_t* cu, int32_t n_docs, int32_t n_chunks, sap_plan_t** out) {
+  if (!cu || !out || n_docs < 1 || n_chunks < 1) return SAP_ERR_INVALID_ARG;
+  if (cu[0] != 0) return SAP_ERR_BAD_CU_SEQLENS;
+  for (int32_t e = 0; e < n_docs; ++e)
+    if (cu[e + 1] < cu[e]) return SAP_ERR_BAD_CU_SEQLENS;
+  const int64_t N = cu[n_docs];
+  if (N <= 0) return SAP_ERR_BAD_CU_SEQLENS;
+  const int32_t P = n_chunks;
+  if (N % P != 0) return SAP_ERR_INDIVISIBLE;
+  sap_plan* p = new (std::nothrow) sap_plan();
+  if (!p) return SAP_ERR_INVALID_ARG;
+  p->n_docs = n_docs; p->n_chunks = P; p->n_tokens = (int32_t)N; p->chunk_len = (int32_t)(N / P);
+  p->cu.assign(cu, cu + n_docs + 1);
+  const int64_t n = p->chunk_len;
+  p->kind_map.assign((size_t)P * P, (uint8_t)SAP_MASK_SKIP);
+  p->chunk_offsets.resize(P + 1);
+  for (int32_t i = 0; i < P; ++i) {
+    p->chunk_offsets[i] = (int32_t)p->items.size();
+    const int64_t r_begin = (int64_t)i * n, r_end = r_begin + n;
+    const int32_t e_first = doc_of(p->cu, r_begin), e_last = doc_of(p->cu, r_end - 1);
+    {  // step 0: the diagonal block
+      sap_item_t im;
+      im.q_chunk = i; im.kv_chunk = i; im.doc_lo = e_first; im.doc_hi = e_last;
+      im.mask_kind = SAP_MASK_DIAG; im.step = 0;
+      im.q_begin = (int32_t)r_begin; im.q_end = (int32_t)r_end;
+      im.kv_begin = (int32_t)r_begin; im.kv_end = (int32_t)r_end;
+      p->items.push_back(im);
+      p->kind_map[(size_t)i * P + i] = (uint8_t)SAP_MASK_DIAG;
+    }
+    const int64_t d_begin = p->cu[e_first], d_end = p->cu[e_first + 1];
+    for (int32_t s = 1; s <= i; ++s) {  // ring order: j = i-1, i-2, ...
+      const int32_t j = i - s;
+      if (d_begin >= (int64_t)(j + 1) * n) break;  // the document does not reach chunk j (nor any earlier one)
+      sap_item_t im;
+      im.q_chunk = i; im.kv_chunk = j; im.doc_lo = e_first; im.doc_hi = e_first;
+      im.mask_kind = SAP_MASK_FULL; im.step = s;
+      im.q_begin = (int32_t)r_begin; im.q_end = (int32_t)std::min<int64_t>(d_end, r_end);
+      im.kv_begin = (int32_t)std::max<int64_t>(d_begin, (int64_t)j * n); im.kv_end = (int32_t)((int64_t)(j + 1) * n);
+      p->items.push_back(im);
+      p->kind_map[(size_t)i * P + j] = (uint8_t)SAP_MASK_FULL;
+    }
+  }
+  p->chunk_offsets[P] = (int32_t)p->items.size();
+  // transposed index (CSR by kv_chunk, item ids ascending) for the backward pass
+  p->kv_offsets.assign(P + 1, 0);
+  for (const sap_item_t& im : p->items) p->kv_offsets[im.kv_chunk + 1]++;
+  for (int32_t j = 0; j < P; ++j) p->kv_offsets[j + 1] += p->kv_offsets[j];
+  p->kv_index.resize(p->items.size());
+  {
+    std::vector<int32_t> fill(p->kv_offsets.begin(), p->kv_offsets.end() - 1);
+    for (int32_t it = 0; it < (int32_t)p->items.size(); ++it) p->kv_index[fill[p->items[it].kv_chunk]++] = it;
+  }
+  for (int32_t e = 0; e < n_docs; ++e) {
+    const int64_t L = (int64_t)cu[e + 1] - cu[e];
+    p->useful_pairs += L * (L + 1) / 2;
+  }
+  build_q_program(*p, 0, (int32_t)p->items.size(), p->fwd);
+  build_kv_program(*p, p->kv);
+  *out = p;
+  return SAP_OK;
+}
+
+int32_t sap_plan_n_items(const sap_plan_t* p) { return p ? (int32_t)p->items.size() : 0; }
+int32_t sap_plan_n_chunks(const sap_plan_t* p) { return p ? p->n_chunks : 0; }
+int32_t sap_plan_n_tokens(const sap_plan_t* p) { return p ? p->n_tokens : 0; }
+const sap_item_t* sap_plan_items(const sap_plan_t* p) { return p ? p->items.data() : nullptr; }
+const int32_t* sap_plan_chunk_offsets(const sap_plan_t* p) { return p ? p->chunk_offsets.data() : nullptr; }
+const int32_t* sap_plan_kv_offsets(const sap_plan_t* p) { return p ? p->kv_offsets.data() : nullptr; }
+const int32_t* sap_plan_kv_index(const sap_plan_t* p) { return p ? p->kv_index.data() : nullptr; }
+const uint8_t* sap_plan_kind_map(const sap_plan_t* p) { return p ? p->kind_map.data() : nullptr; }
+int64_t sap_plan_useful_pairs(const sap_plan_t* p) { return p ? p->useful_pairs : 0; }
+int64_t sap_plan_fwd_tiles(const sap_plan_t* p) { return p ? p->fwd.streamed_tiles : 0; }
+
+const char* sap_strerror(int status) {
+  switch (status) {
+    case SAP_OK: return "ok";
+    case SAP_ERR_INVALID_ARG: return "invalid argument";
+    case SAP_ERR_BAD_CU_SEQLENS: return "bad cu_seqlens (must start at 0, be non-decreasing, end > 0)";
+    case SAP_ERR_INDIVISIBLE: return "total length is not divisible by n_chunks";
+    case SAP_ERR_UNSUPPORTED: return "unsupported configuration (head_dim in {64,128}, Hq % Hkv == 0, 16-byte aligned pointers)";
+    case SAP_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+    case SAP_ERR_WRONG_ARCH: return "device is not sm_100 (B200)";
+    case SAP_ERR_CUDA: return "CUDA error (see sap_last_cuda_error)";
+    case SAP_ERR_NO_DEVICE: return "no CUDA device";
+    default: return "unknown status";
+  }
+}
+
+}  // extern "C"

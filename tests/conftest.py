@@ -8,7 +8,17 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 
+def _build_native():
+    """Build the C-ABI library and the oracle in-tree when missing or stale (nvcc / g++ cross-compile
+    without a GPU).  Building the oracle is not using it."""
+    from paper_2606_30460_b200 import build as _b
+    _b.build()
+    from oracle import oracle as _o
+    _o.build()
+
+
 def pytest_configure(config):
+    _build_native()
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200, sm_100a)")
     config.addinivalue_line("markers", "slow: long-running parity case")
 
