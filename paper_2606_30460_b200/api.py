@@ -54,9 +54,12 @@ class Plan:
 
     def __del__(self):
         h = getattr(self, "_h", None)
-        if h is not None and h.value:
-            _lib.lib().sap_plan_destroy(h)
-            self._h = ctypes.c_void_p(0)
+        try:
+            if h is not None and h.value:
+                _lib.lib().sap_plan_destroy(h)
+                self._h = ctypes.c_void_p(0)
+        except Exception:      # interpreter shutdown: module globals may already be gone
+            pass
 
     @property
     def handle(self) -> ctypes.c_void_p:

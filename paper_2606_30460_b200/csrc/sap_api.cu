@@ -26,12 +26,12 @@ static EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
-int make_tile_map(CUtensorMap* map, const void* base, int64_t n_rows, int64_t row_elems) {
+int make_tile_map(CUtensorMap* map, const void* base, int64_t n_rows, int64_t row_elems, int box_rows) {
   EncodeTiledFn enc = get_encode_fn();
   if (!enc) { g_last_cuda_error = static_cast<int>(cudaErrorNotSupported); return SAP_ERR_CUDA; }
   cuuint64_t dims[2] = {static_cast<cuuint64_t>(row_elems), static_cast<cuuint64_t>(n_rows)};
   cuuint64_t strides[1] = {static_cast<cuuint64_t>(row_elems) * 2};
-  cuuint32_t box[2] = {64, static_cast<cuuint32_t>(kTile)};
+  cuuint32_t box[2] = {64, static_cast<cuuint32_t>(box_rows)};
   cuuint32_t estr[2] = {1, 1};
   CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -97,6 +97,51 @@ static int launch_fwd(const DevProgram& prog, const void* q, const void* k, cons
   kern<<<grid, kFwdThreads, FwdSmem<D>::kTotal, stream>>>(mq, mk, mv, prog.tiles, prog.segs, cu, plan->n_docs,
                                                           static_cast<__nv_bfloat16*>(out), out_f32, lse,
                                                           plan->n_tokens, Hq, Hkv, scale * kLog2e);
+  g_launch_count.fetch_add(1);
+  SAP_CUDA_CHECK(cudaGetLastError());
+  return SAP_OK;
+}
+
+template <int D>
+static int launch_bwd(const PlanDevice* pd, const void* dout, const void* q, const void* k, const void* v,
+                      const void* out, const float* lse, const int32_t* cu, const sap_plan_t* plan, void* dq, void* dk,
+                      void* dv, int Hq, int Hkv, float scale, float* dsum, cudaStream_t stream) {
+  const int64_t N = plan->n_tokens;
+  int rc;
+  // a5: D = rowsum(dO * O)
+  {
+    const int64_t rows = N * Hq;
+    const int64_t want = (rows * (D / 8) + kPreThreads - 1) / kPreThreads;
+    const unsigned grid = static_cast<unsigned>(want < 148 * 16 ? want : 148 * 16);
+    sap_bwd_pre_kernel<D><<<grid, kPreThreads, 0, stream>>>(static_cast<const __nv_bfloat16*>(dout),
+                                                            static_cast<const __nv_bfloat16*>(out), dsum, N, Hq);
+    g_launch_count.fetch_add(1);
+    SAP_CUDA_CHECK(cudaGetLastError());
+  }
+  CUtensorMap mq128, mdo128, mk64, mv64, mq64, mdo64, mk128, mv128;
+  if ((rc = make_tile_map(&mq128, q, N, (int64_t)Hq * D, kTile)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mdo128, dout, N, (int64_t)Hq * D, kTile)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mk64, k, N, (int64_t)Hkv * D, kBwdN)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mv64, v, N, (int64_t)Hkv * D, kBwdN)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mq64, q, N, (int64_t)Hq * D, kBwdN)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mdo64, dout, N, (int64_t)Hq * D, kBwdN)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mk128, k, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mv128, v, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
+  static bool attr_set = false;
+  if (!attr_set) {
+    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_dq_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, DqSmem<D>::kTotal));
+    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_dkv_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, DkvSmem<D>::kTotal));
+    attr_set = true;
+  }
+  // a6 (dK/dV half first: it is the longer kernel)
+  sap_bwd_dkv_kernel<D><<<static_cast<unsigned>(pd->kv.n_tiles) * Hkv, kDkvThreads, DkvSmem<D>::kTotal, stream>>>(
+      mq64, mdo64, mk128, mv128, pd->kv.tiles, pd->kv.segs, cu, plan->n_docs, lse, dsum,
+      static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
+  g_launch_count.fetch_add(1);
+  SAP_CUDA_CHECK(cudaGetLastError());
+  sap_bwd_dq_kernel<D><<<static_cast<unsigned>(pd->fwd.n_tiles) * Hq, kFwdThreads, DqSmem<D>::kTotal, stream>>>(
+      mq128, mdo128, mk64, mv64, pd->fwd.tiles, pd->fwd.segs, cu, plan->n_docs, lse, dsum,
+      static_cast<__nv_bfloat16*>(dq), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
   g_launch_count.fetch_add(1);
   SAP_CUDA_CHECK(cudaGetLastError());
   return SAP_OK;
@@ -219,10 +264,22 @@ int sap_attn_bwd(const void* dout, const void* q, const void* k, const void* v, 
                  const int32_t* cu_seqlens_dev, sap_plan_t* plan, void* dq, void* dk, void* dv, int n_q_heads,
                  int n_kv_heads, int head_dim, float softmax_scale, void* workspace, size_t workspace_bytes,
                  void* cuda_stream) {
-  (void)dout; (void)q; (void)k; (void)v; (void)out; (void)lse; (void)cu_seqlens_dev; (void)plan; (void)dq; (void)dk;
-  (void)dv; (void)n_q_heads; (void)n_kv_heads; (void)head_dim; (void)softmax_scale; (void)workspace;
-  (void)workspace_bytes; (void)cuda_stream;
-  return SAP_ERR_UNSUPPORTED;
+  if (!dout || !q || !k || !v || !out || !lse || !cu_seqlens_dev || !dq || !dk || !dv) return SAP_ERR_INVALID_ARG;
+  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  if (rc != SAP_OK) return rc;
+  if (!aligned16(dout) || !aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out) || !aligned16(dq) ||
+      !aligned16(dk) || !aligned16(dv) || !aligned16(workspace))
+    return SAP_ERR_UNSUPPORTED;
+  const size_t need = sap_workspace_bytes(plan, n_q_heads, n_kv_heads, head_dim, SAP_PASS_BWD);
+  if (!workspace || workspace_bytes < need) return SAP_ERR_WORKSPACE_TOO_SMALL;
+  if ((rc = sap_plan_upload(plan)) != SAP_OK) return rc;
+  const PlanDevice* pd = static_cast<const PlanDevice*>(plan->dev_state);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (head_dim == 128)
+    return launch_bwd<128>(pd, dout, q, k, v, out, lse, cu_seqlens_dev, plan, dq, dk, dv, n_q_heads, n_kv_heads,
+                           softmax_scale, static_cast<float*>(workspace), st);
+  return launch_bwd<64>(pd, dout, q, k, v, out, lse, cu_seqlens_dev, plan, dq, dk, dv, n_q_heads, n_kv_heads,
+                        softmax_scale, static_cast<float*>(workspace), st);
 }
 
 }  // extern "C"

@@ -40,7 +40,7 @@ int check_device_is_sm100();
 int upload_program(const TileProgram& host, DevProgram& dev);
 void free_program(DevProgram& dev);
 
-// 2D bf16 tensor map over a [n_rows, n_heads*head_dim] matrix, box = 64 columns x 128 rows, 128-byte swizzle.
-int make_tile_map(CUtensorMap* map, const void* base, int64_t n_rows, int64_t row_elems);
+// 2D bf16 tensor map over a [n_rows, n_heads*head_dim] matrix, box = 64 columns x box_rows rows, 128-byte swizzle.
+int make_tile_map(CUtensorMap* map, const void* base, int64_t n_rows, int64_t row_elems, int box_rows = kTile);
 
 }  // namespace sap
