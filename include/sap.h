@@ -142,6 +142,10 @@ const char* sap_strerror(int status);
 int sap_last_cuda_error(void);      /* the cudaError_t / CUresult of the last SAP_ERR_CUDA on this thread */
 /* Number of kernels the library has launched in this process (all streams); for launch accounting. */
 int64_t sap_launch_count(void);
+/* Diagnostic: which kernels sap_attn_bwd launches, so each can be timed alone (bit 0 = D pre-pass,
+ * bit 1 = dK/dV kernel, bit 2 = dQ kernel; default 7 = all).  Process-wide; returns the previous mask.
+ * With a partial mask the skipped outputs are left untouched. */
+int sap_debug_set_bwd_stages(int mask);
 
 #ifdef __cplusplus
 }

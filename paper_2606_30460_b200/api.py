@@ -200,3 +200,8 @@ def sap_attn_bwd(dout, q, k, v, out, lse, cu_seqlens_dev, plan: Plan, softmax_sc
 
 def sap_launch_count() -> int:
     return int(_lib.lib().sap_launch_count())
+
+
+def sap_debug_set_bwd_stages(mask: int) -> int:
+    """Diagnostic: select the kernels sap_attn_bwd launches (1 = D pre-pass, 2 = dK/dV, 4 = dQ)."""
+    return int(_lib.lib().sap_debug_set_bwd_stages(int(mask)))

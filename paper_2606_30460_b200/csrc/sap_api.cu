@@ -11,6 +11,7 @@ namespace sap {
 
 thread_local int g_last_cuda_error = 0;
 std::atomic<int64_t> g_launch_count{0};
+std::atomic<int> g_bwd_stages{7};
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -108,8 +109,9 @@ static int launch_bwd(const PlanDevice* pd, const void* dout, const void* q, con
                       void* dv, int Hq, int Hkv, float scale, float* dsum, cudaStream_t stream) {
   const int64_t N = plan->n_tokens;
   int rc;
+  const int stages = g_bwd_stages.load();
   // a5: D = rowsum(dO * O)
-  {
+  if (stages & 1) {
     const int64_t rows = N * Hq;
     const int64_t want = (rows * (D / 8) + kPreThreads - 1) / kPreThreads;
     const unsigned grid = static_cast<unsigned>(want < 148 * 16 ? want : 148 * 16);
@@ -134,16 +136,20 @@ static int launch_bwd(const PlanDevice* pd, const void* dout, const void* q, con
     attr_set = true;
   }
   // a6 (dK/dV half first: it is the longer kernel)
+  if (stages & 2) {
   sap_bwd_dkv_kernel<D><<<static_cast<unsigned>(pd->kv.n_tiles) * Hkv, kDkvThreads, DkvSmem<D>::kTotal, stream>>>(
       mq64, mdo64, mk128, mv128, pd->kv.tiles, pd->kv.segs, cu, plan->n_docs, lse, dsum,
       static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
   g_launch_count.fetch_add(1);
   SAP_CUDA_CHECK(cudaGetLastError());
+  }
+  if (stages & 4) {
   sap_bwd_dq_kernel<D><<<static_cast<unsigned>(pd->fwd.n_tiles) * Hq, kFwdThreads, DqSmem<D>::kTotal, stream>>>(
       mq128, mdo128, mk64, mv64, pd->fwd.tiles, pd->fwd.segs, cu, plan->n_docs, lse, dsum,
       static_cast<__nv_bfloat16*>(dq), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
   g_launch_count.fetch_add(1);
   SAP_CUDA_CHECK(cudaGetLastError());
+  }
   return SAP_OK;
 }
 
@@ -155,6 +161,7 @@ extern "C" {
 
 int sap_last_cuda_error(void) { return g_last_cuda_error; }
 int64_t sap_launch_count(void) { return g_launch_count.load(); }
+int sap_debug_set_bwd_stages(int mask) { return g_bwd_stages.exchange(mask & 7); }
 
 int sap_plan_upload(sap_plan_t* plan) {
   if (!plan) return SAP_ERR_INVALID_ARG;
