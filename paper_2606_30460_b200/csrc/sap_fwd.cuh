@@ -54,10 +54,10 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const uint32_t sQ = smem_u32(smem), sK = sQ + L::kTileBytes, sV = sK + L::kTileBytes;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L::kBarOffset);
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kBarOffset + 64);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kBarOffset + 96);
   const uint32_t bar_q_full = smem_u32(bars + 0), bar_k_full = smem_u32(bars + 1), bar_k_empty = smem_u32(bars + 2),
                  bar_v_full = smem_u32(bars + 3), bar_v_empty = smem_u32(bars + 4), bar_s_full = smem_u32(bars + 5),
-                 bar_p_full = smem_u32(bars + 6), bar_o_full = smem_u32(bars + 7);
+                 bar_p_full = smem_u32(bars + 6) /* +1: second half of P */, bar_o_full = smem_u32(bars + 8);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int tile_idx = blockIdx.x / n_q_heads, h = blockIdx.x % n_q_heads;
@@ -67,7 +67,7 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
   if (threadIdx.x == 0) {
     mbar_init(bar_q_full, 1); mbar_init(bar_k_full, 1); mbar_init(bar_k_empty, 1);
     mbar_init(bar_v_full, 1); mbar_init(bar_v_empty, 1); mbar_init(bar_s_full, 1);
-    mbar_init(bar_p_full, 128); mbar_init(bar_o_full, 1);
+    mbar_init(bar_p_full, 128); mbar_init(bar_p_full + 8, 128); mbar_init(bar_o_full, 1);
     fence_mbar_init();
     tma_prefetch_desc(&mapQ); tma_prefetch_desc(&mapK); tma_prefetch_desc(&mapV);
   }
@@ -83,6 +83,7 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
 
   if (warp == 0) {
     // ------------------------------------------------------------------ TMA producer
+    reg_dealloc<56>();
     if (lane == 0 && n_iters > 0) {
       mbar_expect_tx(bar_q_full, L::kTileBytes);
 #pragma unroll
@@ -104,6 +105,7 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
     }
   } else if (warp == 1) {
     // ------------------------------------------------------------------ tcgen05 issuer
+    reg_dealloc<56>();
     if (n_iters > 0) {
       constexpr uint32_t idesc_s = make_idesc_bf16(128, 128, 0, 0);  // S[128x128] = Q (K-major) x K^T (K-major)
       constexpr uint32_t idesc_o = make_idesc_bf16(128, D, 0, 1);    // O[128xD]  = P (TMEM)   x V (MN-major)
@@ -121,21 +123,30 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
           umma_commit(bar_s_full);
         }
         __syncwarp();
-        mbar_wait(bar_p_full, it & 1);
         mbar_wait(bar_v_full, it & 1);
-        tc_fence_after();
-        if (lane == 0) {
 #pragma unroll
-          for (int k = 0; k < kTile / 16; ++k)  // 16 keys per MMA: 2 groups of 8 rows (SBO 1024 B); d blocks LBO apart
-            umma_ts(tO, tP + k * 8, make_smem_desc(sV + k * 2048, L::kBoxBytes, 1024), idesc_o, (it > 0 || k > 0) ? 1u : 0u);
-          umma_commit(bar_v_empty);
-          if (it == n_iters - 1) umma_commit(bar_o_full);
+        for (int half = 0; half < 2; ++half) {  // PV starts as soon as the first 64 keys of P are in TMEM
+          mbar_wait(bar_p_full + 8 * half, it & 1);
+          tc_fence_after();
+          if (lane == 0) {
+#pragma unroll
+            for (int k = half * 4; k < half * 4 + 4; ++k)  // 16 keys per MMA: 2 groups of 8 rows (SBO 1024 B); d blocks LBO apart
+              umma_ts(tO, tP + k * 8, make_smem_desc(sV + k * 2048, L::kBoxBytes, 1024), idesc_o, (it > 0 || k > 0) ? 1u : 0u);
+            if (half == 1) {
+              umma_commit(bar_v_empty);
+              if (it == n_iters - 1) umma_commit(bar_o_full);
+            }
+          }
+          __syncwarp();
         }
         __syncwarp();
       }
     }
-  } else if (warp >= 4) {
+  } else if (warp < 4) {
+    reg_dealloc<56>();
+  } else {
     // ------------------------------------------------------------------ softmax / correction / epilogue
+    reg_alloc<200>();
     const int r = (warp - 4) * 32 + lane;
     const int t = td.row0 + r;
     const bool valid = r < td.rows;
@@ -152,25 +163,25 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
         mbar_wait(bar_s_full, it & 1);
         tc_fence_after();
         const bool need_mask = __any_sync(0xffffffffu, (c0 < lo) || (c0 + kTile > hi));
-        // pass 1: row max
-        float mx = -CUDART_INF_F;
+        // the whole S row of this thread: 128 fp32 in registers, one TMEM read
+        uint32_t sv[128];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          uint32_t v[32];
-          tmem_ld32(tS + lane_base + c * 32, v);
-          tmem_wait_ld();
-          if (need_mask) {
+        for (int c = 0; c < 4; ++c) tmem_ld32(tS + lane_base + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[c * 32]));
+        tmem_wait_ld();
+        if (need_mask) {  // boundary tiles only (document start, diagonal, item edge)
 #pragma unroll
-            for (int i = 0; i < 32; ++i) {
-              const int col = c0 + c * 32 + i;
-              mx = fmaxf(mx, (col >= lo && col < hi) ? __uint_as_float(v[i]) : -CUDART_INF_F);
-            }
-          } else {
-#pragma unroll
-            for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(v[i]));
+          for (int i = 0; i < 128; ++i) {
+            const int col = c0 + i;
+            if (!(col >= lo && col < hi)) sv[i] = 0xff800000u;  // -inf
           }
         }
-        const float m_new = mx * scale_log2;
+        float mx4[4] = {-CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F};
+#pragma unroll
+        for (int i = 0; i < 128; i += 4) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) mx4[e] = fmaxf(mx4[e], __uint_as_float(sv[i + e]));
+        }
+        const float m_new = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * scale_log2;
         // lazy rescale: only when the max moved by more than 2^8 (or the row saw its first key)
         const bool grow = m_new > m_used + kRescaleThreshold || (m_used == -CUDART_INF_F && m_new > -CUDART_INF_F);
         if (__any_sync(0xffffffffu, grow)) {
@@ -189,30 +200,27 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
           }
         }
         const float neg_m = (m_used == -CUDART_INF_F) ? 0.f : -m_used;
-        // pass 2: P = 2^(S*scale_log2 - m), row sum, bf16 P back into TMEM over S
+        // P = 2^(S*scale_log2 - m) (masked entries: 2^-inf = 0), row sum, bf16 P back into TMEM over S
+        float ls4[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          uint32_t v[32];
-          tmem_ld32(tS + lane_base + c * 32, v);
-          tmem_wait_ld();
-          uint32_t pk[16];
+        for (int half = 0; half < 2; ++half) {
 #pragma unroll
-          for (int i = 0; i < 32; i += 2) {
-            float p0 = ex2_approx(fmaf(__uint_as_float(v[i]), scale_log2, neg_m));
-            float p1 = ex2_approx(fmaf(__uint_as_float(v[i + 1]), scale_log2, neg_m));
-            if (need_mask) {
-              const int col = c0 + c * 32 + i;
-              if (!(col >= lo && col < hi)) p0 = 0.f;
-              if (!(col + 1 >= lo && col + 1 < hi)) p1 = 0.f;
+          for (int c = half * 2; c < half * 2 + 2; ++c) {
+            uint32_t pk[16];
+#pragma unroll
+            for (int i = 0; i < 32; i += 2) {
+              const float p0 = ex2_approx(fmaf(__uint_as_float(sv[c * 32 + i]), scale_log2, neg_m));
+              const float p1 = ex2_approx(fmaf(__uint_as_float(sv[c * 32 + i + 1]), scale_log2, neg_m));
+              ls4[(i >> 1) & 3] += p0 + p1;
+              pk[i >> 1] = pack_bf16x2(p0, p1);
             }
-            l_run += p0 + p1;
-            pk[i >> 1] = pack_bf16x2(p0, p1);
+            tmem_st16(tP + lane_base + c * 16, pk);
           }
-          tmem_st16(tP + lane_base + c * 16, pk);
+          tmem_wait_st();
+          tc_fence_before();
+          mbar_arrive(bar_p_full + 8 * half);
         }
-        tmem_wait_st();
-        tc_fence_before();
-        mbar_arrive(bar_p_full);
+        l_run += (ls4[0] + ls4[1]) + (ls4[2] + ls4[3]);
       }
     }
     // ---- epilogue: O / l -> global, LSE (natural log, PAPER.md silent: SURVEY A-11)

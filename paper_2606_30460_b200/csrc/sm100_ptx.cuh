@@ -148,6 +148,10 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16
       : "memory");
 }
 
+// Warpgroup register reallocation (all 4 warps of a warpgroup must execute it).
+template <int N> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+
 // ------------------------------------------------------------------ UMMA descriptors
 // Shared-memory matrix descriptor (64 bit), sm_100 format:
 //   [0,14) start address >> 4      [16,30) leading byte offset >> 4   [32,46) stride byte offset >> 4
