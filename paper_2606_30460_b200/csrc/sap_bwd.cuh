@@ -101,8 +101,8 @@ sap_bwd_dq_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kBarOffset + 128);
   const uint32_t bar_q_full = smem_u32(bars + 0), bar_k_full = smem_u32(bars + 1) /* +1: stage 1 */,
                  bar_k_empty = smem_u32(bars + 3) /* +1 */, bar_v_full = smem_u32(bars + 5),
-                 bar_v_empty = smem_u32(bars + 6), bar_s_full = smem_u32(bars + 7), bar_ds_full = smem_u32(bars + 8),
-                 bar_dq_full = smem_u32(bars + 9);
+                 bar_v_empty = smem_u32(bars + 6), bar_s_full = smem_u32(bars + 7), bar_ds_full = smem_u32(bars + 8) /* +1 */,
+                 bar_dq_full = smem_u32(bars + 10);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int tile_idx = blockIdx.x / n_q_heads, h = blockIdx.x % n_q_heads;
@@ -114,7 +114,7 @@ sap_bwd_dq_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
     mbar_init(bar_k_full, 1); mbar_init(bar_k_full + 8, 1);
     mbar_init(bar_k_empty, 1); mbar_init(bar_k_empty + 8, 1);
     mbar_init(bar_v_full, 1); mbar_init(bar_v_empty, 1); mbar_init(bar_s_full, 1);
-    mbar_init(bar_ds_full, 128); mbar_init(bar_dq_full, 1);
+    mbar_init(bar_ds_full, 128); mbar_init(bar_ds_full + 8, 128); mbar_init(bar_dq_full, 1);
     fence_mbar_init();
     tma_prefetch_desc(&mapQ); tma_prefetch_desc(&mapDO); tma_prefetch_desc(&mapK); tma_prefetch_desc(&mapV);
   }
@@ -132,6 +132,7 @@ sap_bwd_dq_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
   }
 
   if (warp == 0) {
+    reg_dealloc<56>();
     if (lane == 0 && n_iters > 0) {
       mbar_expect_tx(bar_q_full, 2 * L::kQBytes);
 #pragma unroll
@@ -157,6 +158,7 @@ sap_bwd_dq_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
       }
     }
   } else if (warp == 1) {
+    reg_dealloc<56>();
     if (n_iters > 0) {
       constexpr uint32_t idesc_s = make_idesc_bf16(128, kBwdN, 0, 0);  // S, dP [128x64]: K-major x K-major
       constexpr uint32_t idesc_dq = make_idesc_bf16(128, D, 0, 1);     // dQ [128xD] = dS (TMEM) x K (MN-major)
@@ -182,19 +184,27 @@ sap_bwd_dq_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
           umma_commit(bar_s_full);
         }
         __syncwarp();
-        mbar_wait(bar_ds_full, it & 1);
-        tc_fence_after();
-        if (lane == 0) {
 #pragma unroll
-          for (int k = 0; k < kBwdN / 16; ++k)
-            umma_ts(tDQ, tDS + k * 8, make_smem_desc(sKs + k * 2048, L::kKBox, 1024), idesc_dq, (it > 0 || k > 0) ? 1u : 0u);
-          umma_commit(bar_k_empty + 8 * st);
-          if (it == n_iters - 1) umma_commit(bar_dq_full);
+        for (int half = 0; half < 2; ++half) {  // dQ starts as soon as the first 32 keys of dS are in TMEM
+          mbar_wait(bar_ds_full + 8 * half, it & 1);
+          tc_fence_after();
+          if (lane == 0) {
+#pragma unroll
+            for (int k = half * 2; k < half * 2 + 2; ++k)
+              umma_ts(tDQ, tDS + k * 8, make_smem_desc(sKs + k * 2048, L::kKBox, 1024), idesc_dq, (it > 0 || k > 0) ? 1u : 0u);
+            if (half == 1) {
+              umma_commit(bar_k_empty + 8 * st);
+              if (it == n_iters - 1) umma_commit(bar_dq_full);
+            }
+          }
+          __syncwarp();
         }
-        __syncwarp();
       }
     }
-  } else if (warp >= 4) {
+  } else if (warp < 4) {
+    reg_dealloc<56>();
+  } else {
+    reg_alloc<200>();
     const int r = (warp - 4) * 32 + lane;
     const int t = td.row0 + r;
     const bool valid = r < td.rows;
@@ -211,29 +221,35 @@ sap_bwd_dq_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
         mbar_wait(bar_s_full, it & 1);
         tc_fence_after();
         const bool need_mask = __any_sync(0xffffffffu, (c0 < lo) || (c0 + kBwdN > hi));
+        uint32_t sv[64], dp[64];
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
-          uint32_t sv[32], dp[32];
-          tmem_ld32(tS + lane_base + c * 32, sv);
-          tmem_ld32(tDP + lane_base + c * 32, dp);
-          tmem_wait_ld();
+          tmem_ld32(tS + lane_base + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[c * 32]));
+          tmem_ld32(tDP + lane_base + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&dp[c * 32]));
+        }
+        tmem_wait_ld();
+        if (need_mask) {  // boundary tiles only: masked scores become -inf => P = 0 => dS = 0
+#pragma unroll
+          for (int i = 0; i < 64; ++i) {
+            const int col = c0 + i;
+            if (!(col >= lo && col < hi)) sv[i] = 0xff800000u;
+          }
+        }
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
           uint32_t pk[16];
 #pragma unroll
           for (int i = 0; i < 32; i += 2) {
-            float p0 = ex2_approx(fmaf(__uint_as_float(sv[i]), scale_log2, -lse2));
-            float p1 = ex2_approx(fmaf(__uint_as_float(sv[i + 1]), scale_log2, -lse2));
-            if (need_mask) {
-              const int col = c0 + c * 32 + i;
-              if (!(col >= lo && col < hi)) p0 = 0.f;
-              if (!(col + 1 >= lo && col + 1 < hi)) p1 = 0.f;
-            }
-            pk[i >> 1] = pack_bf16x2(p0 * (__uint_as_float(dp[i]) - dsum_t), p1 * (__uint_as_float(dp[i + 1]) - dsum_t));
+            const float p0 = ex2_approx(fmaf(__uint_as_float(sv[c * 32 + i]), scale_log2, -lse2));
+            const float p1 = ex2_approx(fmaf(__uint_as_float(sv[c * 32 + i + 1]), scale_log2, -lse2));
+            pk[i >> 1] = pack_bf16x2(p0 * (__uint_as_float(dp[c * 32 + i]) - dsum_t),
+                                     p1 * (__uint_as_float(dp[c * 32 + i + 1]) - dsum_t));
           }
           tmem_st16(tDS + lane_base + c * 16, pk);
+          tmem_wait_st();
+          tc_fence_before();
+          mbar_arrive(bar_ds_full + 8 * c);
         }
-        tmem_wait_st();
-        tc_fence_before();
-        mbar_arrive(bar_ds_full);
       }
     }
     if (n_iters > 0) {
@@ -370,8 +386,9 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         }
       }
     }
-  } else if (warp == 2) {
-    // ------------------------------------------------------------------ per-row LSE (log2 domain) and D loader
+  } else if (warp == 2 || warp == 3) {
+    // ------------------------------------------------------------------ per-row LSE (log2 domain) and D loaders
+    // two warps take alternate iterations, so each has two iteration times to cover the global-load latency
     int i = 0;
     for (int hq = 0; hq < g; ++hq) {
       const int h = hk * g + hq;
@@ -380,6 +397,7 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       for (int s = td.seg_begin; s < td.seg_end; ++s) {
         const int t_begin = segs[s].t_begin, t_end = segs[s].t_end;
         for (int t0 = t_begin; t0 < t_end; t0 += kBwdN, ++i) {
+          if ((i & 1) != (warp & 1)) continue;
           const int st = i % kDkvStages;
           float a[2], b[2];
 #pragma unroll
@@ -478,6 +496,13 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
           const float4* l4 = reinterpret_cast<const float4*>(stat + st * 128 + 32 * half);
           const float4* d4 = reinterpret_cast<const float4*>(stat + st * 128 + 64 + 32 * half);
           tmem_wait_ld();
+          if (need_mask) {  // boundary tiles only: masked scores become -inf, so P = 2^-inf = 0 and dS = 0
+#pragma unroll
+            for (int idx = 0; idx < 32; ++idx) {
+              const int t = tc + idx;
+              if (!(t >= lo && t < hi)) sv[idx] = 0xff800000u;
+            }
+          }
           uint32_t pk[16], dsk[16];
 #pragma unroll
           for (int q4 = 0; q4 < 8; ++q4) {
@@ -488,10 +513,6 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             for (int e = 0; e < 4; ++e) {
               const int idx = q4 * 4 + e;
               p[e] = ex2_approx(fmaf(__uint_as_float(sv[idx]), scale_log2, -ls[e]));
-              if (need_mask) {
-                const int t = tc + idx;
-                if (!(t >= lo && t < hi)) p[e] = 0.f;
-              }
               ds[e] = p[e] * (__uint_as_float(dp[idx]) - dd[e]);
             }
             pk[q4 * 2] = pack_bf16x2(p[0], p[1]); pk[q4 * 2 + 1] = pack_bf16x2(p[2], p[3]);
