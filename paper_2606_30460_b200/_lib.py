@@ -6,7 +6,7 @@ import ctypes
 import os
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libsap_b200.so")
+LIB_PATH = os.environ.get("SAP_B200_LIB", os.path.join(HERE, "libsap_b200.so"))  # override: instrumented builds
 
 c_i32p = ctypes.POINTER(ctypes.c_int32)
 c_f32p = ctypes.POINTER(ctypes.c_float)

@@ -66,6 +66,13 @@ __device__ __forceinline__ int32_t doc_end_of(const int32_t* __restrict__ cu, in
 
 constexpr int kBwdN = 64;  // streamed tile rows in both backward kernels
 
+#ifdef SAP_TRACE  // instrumented build only (never the shipped library): SM cycle stamps of one CTA
+__device__ unsigned long long g_sap_trace[128 * 16];
+#define SAP_STAMP(iter, slot) do { if (blockIdx.x == 0 && (iter) < 128) g_sap_trace[(iter) * 16 + (slot)] = clock64(); } while (0)
+#else
+#define SAP_STAMP(iter, slot) do { } while (0)
+#endif
+
 // ------------------------------------------------------------------------------------------------
 // dQ kernel.  One CTA = one 128-row Q tile x one q-head, two CTAs per SM (same recipe as the forward).
 // TMEM (256 columns): [0,64) S fp32 -> dS bf16 in [0,32); [64,128) dP fp32; [128,128+D) dQ fp32.
@@ -133,7 +140,7 @@ sap_bwd_dq_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
 
   if (warp == 0) {
     reg_dealloc<56>();
-    if (lane == 0 && n_iters > 0) {
+    if (n_iters > 0 && elect_one()) {
       mbar_expect_tx(bar_q_full, 2 * L::kQBytes);
 #pragma unroll
       for (int b = 0; b < L::kBoxes; ++b) {
@@ -169,7 +176,7 @@ sap_bwd_dq_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
         mbar_wait(bar_k_full + 8 * st, (it >> 1) & 1);
         mbar_wait(bar_v_full, it & 1);
         tc_fence_after();
-        if (lane == 0) {
+        if (elect_one()) {
 #pragma unroll
           for (int k = 0; k < D / 16; ++k) {
             const uint32_t offq = (k / 4) * L::kQBox + (k % 4) * 32, offk = (k / 4) * L::kKBox + (k % 4) * 32;
@@ -188,7 +195,7 @@ sap_bwd_dq_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
         for (int half = 0; half < 2; ++half) {  // dQ starts as soon as the first 32 keys of dS are in TMEM
           mbar_wait(bar_ds_full + 8 * half, it & 1);
           tc_fence_after();
-          if (lane == 0) {
+          if (elect_one()) {
 #pragma unroll
             for (int k = half * 2; k < half * 2 + 2; ++k)
               umma_ts(tDQ, tDS + k * 8, make_smem_desc(sKs + k * 2048, L::kKBox, 1024), idesc_dq, (it > 0 || k > 0) ? 1u : 0u);
@@ -361,7 +368,7 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
 
   if (warp == 0) {
     // ------------------------------------------------------------------ TMA producer
-    if (lane == 0 && n_iters > 0) {
+    if (n_iters > 0 && elect_one()) {
       mbar_expect_tx(bar_kv_full, 2 * L::kKVBytes);
 #pragma unroll
       for (int b = 0; b < L::kBoxes; ++b) {
@@ -427,9 +434,11 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
           const int st = i % kDkvStages, b = i & 1;
           const uint32_t sQs = sQ + st * L::kQBytes, sDOs = sDO + st * L::kQBytes;
           const uint32_t tST = tBuf + 128 * b, tDPT = tST + 64;
+          if (lane == 0) SAP_STAMP(i, 0);
           mbar_wait(bar_qdo_full + 8 * st, (i / kDkvStages) & 1);
           tc_fence_after();
-          if (lane == 0) {
+          if (elect_one()) {
+            SAP_STAMP(i, 1);
 #pragma unroll
             for (int k = 0; k < D / 16; ++k) {
               const uint32_t offk = (k / 4) * L::kKVBox + (k % 4) * 32, offq = (k / 4) * L::kQBox + (k % 4) * 32;
@@ -441,6 +450,7 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
               umma_ss(tDPT, make_smem_desc(sV + offk, 16, 1024), make_smem_desc(sDOs + offq, 16, 1024), idesc_s, k > 0);
             }
             umma_commit(bar_s_full + 8 * b);
+            SAP_STAMP(i, 2);
           }
           __syncwarp();
         }
@@ -450,7 +460,8 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
           const uint32_t tPT = tBuf + 128 * b, tDST = tPT + 64;
           mbar_wait(bar_p_full + 8 * b, (j >> 1) & 1);
           tc_fence_after();
-          if (lane == 0) {
+          if (elect_one()) {
+            SAP_STAMP(j, 3);
 #pragma unroll
             for (int k = 0; k < kBwdN / 16; ++k) {  // k-steps 0,1 live in columns [0,16), 2,3 in [32,48)
               const uint32_t acol = (k >> 1) * 32 + (k & 1) * 8;
@@ -462,6 +473,7 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
               umma_ts(tDK, tDST + acol, make_smem_desc(sQs + k * 2048, L::kQBox, 1024), idesc_acc, (j > 0 || k > 0) ? 1u : 0u);
             }
             umma_commit(bar_qdo_empty + 8 * st);
+            SAP_STAMP(j, 4);
             if (j == n_iters - 1) umma_commit(bar_acc_full);
           }
           __syncwarp();
@@ -486,9 +498,12 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
           const int st = i % kDkvStages, b = i & 1;
           const uint32_t tST = tBuf + 128 * b + lane_base, tDPT = tST + 64;
           const int tc = t0 + 32 * half;  // first q row of this warp's column half
+          if (threadIdx.x == 128) SAP_STAMP(i, 8);
           mbar_wait(bar_stat_full + 8 * st, (i / kDkvStages) & 1);
+          if (threadIdx.x == 128) SAP_STAMP(i, 9);
           mbar_wait(bar_s_full + 8 * b, (i >> 1) & 1);
           tc_fence_after();
+          if (threadIdx.x == 128) SAP_STAMP(i, 10);
           const bool need_mask = __any_sync(0xffffffffu, (tc < lo) || (tc + 32 > hi));
           uint32_t sv[32], dp[32];
           tmem_ld32(tST + 32 * half, sv);
@@ -496,6 +511,7 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
           const float4* l4 = reinterpret_cast<const float4*>(stat + st * 128 + 32 * half);
           const float4* d4 = reinterpret_cast<const float4*>(stat + st * 128 + 64 + 32 * half);
           tmem_wait_ld();
+          if (threadIdx.x == 128) SAP_STAMP(i, 11);
           if (need_mask) {  // boundary tiles only: masked scores become -inf, so P = 2^-inf = 0 and dS = 0
 #pragma unroll
             for (int idx = 0; idx < 32; ++idx) {
@@ -518,10 +534,12 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             pk[q4 * 2] = pack_bf16x2(p[0], p[1]); pk[q4 * 2 + 1] = pack_bf16x2(p[2], p[3]);
             dsk[q4 * 2] = pack_bf16x2(ds[0], ds[1]); dsk[q4 * 2 + 1] = pack_bf16x2(ds[2], ds[3]);
           }
+          if (threadIdx.x == 128) SAP_STAMP(i, 12);
           tmem_st16(tST + 32 * half, pk);
           tmem_st16(tDPT + 32 * half, dsk);
           tmem_wait_st();
           tc_fence_before();
+          if (threadIdx.x == 128) SAP_STAMP(i, 13);
           mbar_arrive(bar_p_full + 8 * b);
           mbar_arrive(bar_stat_empty + 8 * st);
         }

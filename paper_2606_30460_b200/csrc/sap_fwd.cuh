@@ -84,7 +84,7 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
   if (warp == 0) {
     // ------------------------------------------------------------------ TMA producer
     reg_dealloc<56>();
-    if (lane == 0 && n_iters > 0) {
+    if (n_iters > 0 && elect_one()) {
       mbar_expect_tx(bar_q_full, L::kTileBytes);
 #pragma unroll
       for (int b = 0; b < L::kBoxes; ++b) tma_load_2d(sQ + b * L::kBoxBytes, &mapQ, h * D + b * 64, td.row0, bar_q_full);
@@ -113,7 +113,7 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
       for (int it = 0; it < n_iters; ++it) {
         mbar_wait(bar_k_full, it & 1);
         tc_fence_after();
-        if (lane == 0) {
+        if (elect_one()) {
 #pragma unroll
           for (int k = 0; k < D / 16; ++k) {
             const uint32_t off = (k / 4) * L::kBoxBytes + (k % 4) * 32;
@@ -128,7 +128,7 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
         for (int half = 0; half < 2; ++half) {  // PV starts as soon as the first 64 keys of P are in TMEM
           mbar_wait(bar_p_full + 8 * half, it & 1);
           tc_fence_after();
-          if (lane == 0) {
+          if (elect_one()) {
 #pragma unroll
             for (int k = half * 4; k < half * 4 + 4; ++k)  // 16 keys per MMA: 2 groups of 8 rows (SBO 1024 B); d blocks LBO apart
               umma_ts(tO, tP + k * 8, make_smem_desc(sV + k * 2048, L::kBoxBytes, 1024), idesc_o, (it > 0 || k > 0) ? 1u : 0u);
