@@ -163,7 +163,7 @@ int sap_last_cuda_error(void) { return g_last_cuda_error; }
 int64_t sap_launch_count(void) { return g_launch_count.load(); }
 #ifdef SAP_TRACE
 int sap_debug_read_trace(unsigned long long* host_out) {
-  return (int)cudaMemcpyFromSymbol(host_out, g_sap_trace, sizeof(unsigned long long) * 128 * 16);
+  return (int)cudaMemcpyFromSymbol(host_out, g_sap_trace, sizeof(unsigned long long) * 128 * 64);
 }
 #endif
 int sap_debug_set_bwd_stages(int mask) { return g_bwd_stages.exchange(mask & 7); }

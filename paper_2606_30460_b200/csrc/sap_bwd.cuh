@@ -67,8 +67,8 @@ __device__ __forceinline__ int32_t doc_end_of(const int32_t* __restrict__ cu, in
 constexpr int kBwdN = 64;  // streamed tile rows in both backward kernels
 
 #ifdef SAP_TRACE  // instrumented build only (never the shipped library): SM cycle stamps of one CTA
-__device__ unsigned long long g_sap_trace[128 * 16];
-#define SAP_STAMP(iter, slot) do { if (blockIdx.x == 0 && (iter) < 128) g_sap_trace[(iter) * 16 + (slot)] = clock64(); } while (0)
+__device__ unsigned long long g_sap_trace[128 * 64];
+#define SAP_STAMP(iter, slot) do { if (blockIdx.x == 0 && (iter) < 128) g_sap_trace[(iter) * 64 + (slot)] = clock64(); } while (0)
 #else
 #define SAP_STAMP(iter, slot) do { } while (0)
 #endif
@@ -111,7 +111,10 @@ sap_bwd_dq_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
                  bar_v_empty = smem_u32(bars + 6), bar_s_full = smem_u32(bars + 7), bar_ds_full = smem_u32(bars + 8) /* +1 */,
                  bar_dq_full = smem_u32(bars + 10);
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // logical warp id: the service warps (0-3: TMA, tcgen05 issuer, ...) are the physically LAST four warps, because the
+  // SM's warp arbiter favours high warp ids and the single issuing threads must never starve; +4 keeps warp % 4
+  // (the TMEM lane quarter) and the warpgroup split of setmaxnreg intact
+  const int warp = ((threadIdx.x >> 5) + 4) & 7, lane = threadIdx.x & 31;
   const int tile_idx = blockIdx.x / n_q_heads, h = blockIdx.x % n_q_heads;
   const int hk = h / (n_q_heads / n_kv_heads);
   const TileDesc td = tiles[tile_idx];
@@ -302,7 +305,9 @@ sap_bwd_dq_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
 //   P^T bf16 written over columns [32h, 32h+16) by the warp of half h; dP^T fp32 [64,128), dS^T likewise.
 // The issuer runs one iteration ahead: S^T/dP^T of tile i+1 are in flight while tile i is in softmax.
 // ------------------------------------------------------------------------------------------------
-constexpr int kDkvThreads = 384;
+constexpr int kDkvParts = 4;                        // column parts of the 64 streamed q rows, one compute warp each
+constexpr int kDkvThreads = 128 + 128 * kDkvParts;  // 4 service warps + 4 * kDkvParts compute warps
+constexpr int kDkvCols = kBwdN / kDkvParts;        // q rows (TMEM columns) per compute warp
 constexpr int kDkvStages = 3;
 
 template <int D>
@@ -339,7 +344,8 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                  bar_stat_full = smem_u32(bars + 7), bar_stat_empty = smem_u32(bars + 10),
                  bar_s_full = smem_u32(bars + 13), bar_p_full = smem_u32(bars + 15), bar_acc_full = smem_u32(bars + 17);
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // logical warp id: service warps (0-3) are the physically last four (see sap_fwd.cuh)
+  const int warp = ((threadIdx.x >> 5) + 4) % (kDkvThreads / 32), lane = threadIdx.x & 31;
   const int tile_idx = blockIdx.x / n_kv_heads, hk = blockIdx.x % n_kv_heads;
   const int g = n_q_heads / n_kv_heads;
   const TileDesc td = tiles[tile_idx];
@@ -348,9 +354,9 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     mbar_init(bar_kv_full, 1);
     for (int i = 0; i < kDkvStages; ++i) {
       mbar_init(bar_qdo_full + 8 * i, 1); mbar_init(bar_qdo_empty + 8 * i, 1);
-      mbar_init(bar_stat_full + 8 * i, 32); mbar_init(bar_stat_empty + 8 * i, 256);
+      mbar_init(bar_stat_full + 8 * i, 32); mbar_init(bar_stat_empty + 8 * i, 128 * kDkvParts);
     }
-    for (int i = 0; i < 2; ++i) { mbar_init(bar_s_full + 8 * i, 1); mbar_init(bar_p_full + 8 * i, 256); }
+    for (int i = 0; i < 2; ++i) { mbar_init(bar_s_full + 8 * i, 1); mbar_init(bar_p_full + 8 * i, 128 * kDkvParts); }
     mbar_init(bar_acc_full, 1);
     fence_mbar_init();
     tma_prefetch_desc(&mapQ); tma_prefetch_desc(&mapDO); tma_prefetch_desc(&mapK); tma_prefetch_desc(&mapV);
@@ -424,65 +430,59 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       }
     }
   } else if (warp == 1) {
-    // ------------------------------------------------------------------ tcgen05 issuer
-    if (n_iters > 0) {
+    // ------------------------------------------------------------------ tcgen05 issuer: one elected thread runs
+    // the whole loop (no per-iteration warp sync / election); stage and phase counters are incremental
+    if (n_iters > 0 && elect_one()) {
       constexpr uint32_t idesc_s = make_idesc_bf16(128, kBwdN, 0, 0);  // S^T, dP^T [128x64]: K-major x K-major
       constexpr uint32_t idesc_acc = make_idesc_bf16(128, D, 0, 1);    // dV, dK [128xD]: TMEM x MN-major
+      const uint64_t dK0 = make_smem_desc(sK, 16, 1024), dV0 = make_smem_desc(sV, 16, 1024);
+      const uint64_t dQk0 = make_smem_desc(sQ, 16, 1024), dDOk0 = make_smem_desc(sDO, 16, 1024);          // K-major views
+      const uint64_t dQm0 = make_smem_desc(sQ, L::kQBox, 1024), dDOm0 = make_smem_desc(sDO, L::kQBox, 1024);  // MN-major views
       mbar_wait(bar_kv_full, 0);
+      int st_i = 0, ph_i = 0, st_j = 0;
       for (int i = 0; i <= n_iters; ++i) {
         if (i < n_iters) {
-          const int st = i % kDkvStages, b = i & 1;
-          const uint32_t sQs = sQ + st * L::kQBytes, sDOs = sDO + st * L::kQBytes;
+          const int b = i & 1;
           const uint32_t tST = tBuf + 128 * b, tDPT = tST + 64;
-          if (lane == 0) SAP_STAMP(i, 0);
-          mbar_wait(bar_qdo_full + 8 * st, (i / kDkvStages) & 1);
+          SAP_STAMP(i, 0);
+          mbar_wait(bar_qdo_full + 8 * st_i, ph_i);
           tc_fence_after();
-          if (elect_one()) {
-            SAP_STAMP(i, 1);
+          SAP_STAMP(i, 1);
+          const uint64_t dq = desc_add(dQk0, st_i * L::kQBytes), ddo = desc_add(dDOk0, st_i * L::kQBytes);
 #pragma unroll
-            for (int k = 0; k < D / 16; ++k) {
-              const uint32_t offk = (k / 4) * L::kKVBox + (k % 4) * 32, offq = (k / 4) * L::kQBox + (k % 4) * 32;
-              umma_ss(tST, make_smem_desc(sK + offk, 16, 1024), make_smem_desc(sQs + offq, 16, 1024), idesc_s, k > 0);
-            }
+          for (int k = 0; k < D / 16; ++k)
+            umma_ss(tST, desc_add(dK0, (k / 4) * L::kKVBox + (k % 4) * 32), desc_add(dq, (k / 4) * L::kQBox + (k % 4) * 32), idesc_s, k > 0);
 #pragma unroll
-            for (int k = 0; k < D / 16; ++k) {
-              const uint32_t offk = (k / 4) * L::kKVBox + (k % 4) * 32, offq = (k / 4) * L::kQBox + (k % 4) * 32;
-              umma_ss(tDPT, make_smem_desc(sV + offk, 16, 1024), make_smem_desc(sDOs + offq, 16, 1024), idesc_s, k > 0);
-            }
-            umma_commit(bar_s_full + 8 * b);
-            SAP_STAMP(i, 2);
-          }
-          __syncwarp();
+          for (int k = 0; k < D / 16; ++k)
+            umma_ss(tDPT, desc_add(dV0, (k / 4) * L::kKVBox + (k % 4) * 32), desc_add(ddo, (k / 4) * L::kQBox + (k % 4) * 32), idesc_s, k > 0);
+          umma_commit(bar_s_full + 8 * b);
+          SAP_STAMP(i, 2);
+          if (++st_i == kDkvStages) { st_i = 0; ph_i ^= 1; }
         }
         if (i > 0) {
-          const int j = i - 1, st = j % kDkvStages, b = j & 1;
-          const uint32_t sQs = sQ + st * L::kQBytes, sDOs = sDO + st * L::kQBytes;
+          const int j = i - 1, b = j & 1;
           const uint32_t tPT = tBuf + 128 * b, tDST = tPT + 64;
+          SAP_STAMP(j, 5);
           mbar_wait(bar_p_full + 8 * b, (j >> 1) & 1);
           tc_fence_after();
-          if (elect_one()) {
-            SAP_STAMP(j, 3);
+          SAP_STAMP(j, 3);
+          const uint64_t dq = desc_add(dQm0, st_j * L::kQBytes), ddo = desc_add(dDOm0, st_j * L::kQBytes);
 #pragma unroll
-            for (int k = 0; k < kBwdN / 16; ++k) {  // k-steps 0,1 live in columns [0,16), 2,3 in [32,48)
-              const uint32_t acol = (k >> 1) * 32 + (k & 1) * 8;
-              umma_ts(tDV, tPT + acol, make_smem_desc(sDOs + k * 2048, L::kQBox, 1024), idesc_acc, (j > 0 || k > 0) ? 1u : 0u);
-            }
+          for (int k = 0; k < kBwdN / 16; ++k)  // the bf16 of q rows [16k,16k+16) sit in the 8 columns at 16k
+            umma_ts(tDV, tPT + k * 16, desc_add(ddo, k * 2048), idesc_acc, (j > 0 || k > 0) ? 1u : 0u);
 #pragma unroll
-            for (int k = 0; k < kBwdN / 16; ++k) {
-              const uint32_t acol = (k >> 1) * 32 + (k & 1) * 8;
-              umma_ts(tDK, tDST + acol, make_smem_desc(sQs + k * 2048, L::kQBox, 1024), idesc_acc, (j > 0 || k > 0) ? 1u : 0u);
-            }
-            umma_commit(bar_qdo_empty + 8 * st);
-            SAP_STAMP(j, 4);
-            if (j == n_iters - 1) umma_commit(bar_acc_full);
-          }
-          __syncwarp();
+          for (int k = 0; k < kBwdN / 16; ++k)
+            umma_ts(tDK, tDST + k * 16, desc_add(dq, k * 2048), idesc_acc, (j > 0 || k > 0) ? 1u : 0u);
+          umma_commit(bar_qdo_empty + 8 * st_j);
+          SAP_STAMP(j, 4);
+          if (j == n_iters - 1) umma_commit(bar_acc_full);
+          if (++st_j == kDkvStages) st_j = 0;
         }
       }
     }
   } else if (warp >= 4) {
     // ------------------------------------------------------------------ compute: P^T, dS^T; epilogue
-    const int quarter = warp & 3, half = (warp - 4) >> 2;
+    const int quarter = warp & 3, part = (warp - 4) >> 2;
     const int r = quarter * 32 + lane;
     const int srow = td.row0 + r;                        // key index owned by this thread
     const bool valid = r < td.rows;
@@ -496,32 +496,32 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         if (!valid || srow < sd.kv_lo || srow >= sd.kv_hi) { lo = 0; hi = 0; }
         for (int t0 = sd.t_begin; t0 < sd.t_end; t0 += kBwdN, ++i) {
           const int st = i % kDkvStages, b = i & 1;
-          const uint32_t tST = tBuf + 128 * b + lane_base, tDPT = tST + 64;
-          const int tc = t0 + 32 * half;  // first q row of this warp's column half
-          if (threadIdx.x == 128) SAP_STAMP(i, 8);
+          const uint32_t tST = tBuf + 128 * b + lane_base + kDkvCols * part, tDPT = tST + 64;
+          const int tc = t0 + kDkvCols * part;  // first q row of this warp's column part
+          if (warp == 4 && lane == 0) SAP_STAMP(i, 8);
           mbar_wait(bar_stat_full + 8 * st, (i / kDkvStages) & 1);
-          if (threadIdx.x == 128) SAP_STAMP(i, 9);
+          if (warp == 4 && lane == 0) SAP_STAMP(i, 9);
           mbar_wait(bar_s_full + 8 * b, (i >> 1) & 1);
           tc_fence_after();
-          if (threadIdx.x == 128) SAP_STAMP(i, 10);
-          const bool need_mask = __any_sync(0xffffffffu, (tc < lo) || (tc + 32 > hi));
-          uint32_t sv[32], dp[32];
-          tmem_ld32(tST + 32 * half, sv);
-          tmem_ld32(tDPT + 32 * half, dp);
-          const float4* l4 = reinterpret_cast<const float4*>(stat + st * 128 + 32 * half);
-          const float4* d4 = reinterpret_cast<const float4*>(stat + st * 128 + 64 + 32 * half);
+          if (lane == 0) SAP_STAMP(i, 16 + warp - 4);
+          const bool need_mask = __any_sync(0xffffffffu, (tc < lo) || (tc + kDkvCols > hi));
+          uint32_t sv[kDkvCols], dp[kDkvCols];
+          tmem_ld16(tST, sv);
+          tmem_ld16(tDPT, dp);
+          const float4* l4 = reinterpret_cast<const float4*>(stat + st * 128 + kDkvCols * part);
+          const float4* d4 = reinterpret_cast<const float4*>(stat + st * 128 + 64 + kDkvCols * part);
           tmem_wait_ld();
-          if (threadIdx.x == 128) SAP_STAMP(i, 11);
+          if (warp == 4 && lane == 0) SAP_STAMP(i, 11);
           if (need_mask) {  // boundary tiles only: masked scores become -inf, so P = 2^-inf = 0 and dS = 0
 #pragma unroll
-            for (int idx = 0; idx < 32; ++idx) {
+            for (int idx = 0; idx < kDkvCols; ++idx) {
               const int t = tc + idx;
               if (!(t >= lo && t < hi)) sv[idx] = 0xff800000u;
             }
           }
-          uint32_t pk[16], dsk[16];
+          uint32_t pk[kDkvCols / 2], dsk[kDkvCols / 2];
 #pragma unroll
-          for (int q4 = 0; q4 < 8; ++q4) {
+          for (int q4 = 0; q4 < kDkvCols / 4; ++q4) {
             const float4 lv = l4[q4], dvv = d4[q4];
             const float ls[4] = {lv.x, lv.y, lv.z, lv.w}, dd[4] = {dvv.x, dvv.y, dvv.z, dvv.w};
             float p[4], ds[4];
@@ -534,12 +534,12 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             pk[q4 * 2] = pack_bf16x2(p[0], p[1]); pk[q4 * 2 + 1] = pack_bf16x2(p[2], p[3]);
             dsk[q4 * 2] = pack_bf16x2(ds[0], ds[1]); dsk[q4 * 2 + 1] = pack_bf16x2(ds[2], ds[3]);
           }
-          if (threadIdx.x == 128) SAP_STAMP(i, 12);
-          tmem_st16(tST + 32 * half, pk);
-          tmem_st16(tDPT + 32 * half, dsk);
+          if (lane == 0) SAP_STAMP(i, 48 + warp - 4);
+          tmem_st8(tST, pk);     // bf16 P^T over the S^T columns this warp has just read
+          tmem_st8(tDPT, dsk);   // bf16 dS^T over its dP^T columns
           tmem_wait_st();
           tc_fence_before();
-          if (threadIdx.x == 128) SAP_STAMP(i, 13);
+          if (lane == 0) SAP_STAMP(i, 32 + warp - 4);
           mbar_arrive(bar_p_full + 8 * b);
           mbar_arrive(bar_stat_empty + 8 * st);
         }
@@ -549,12 +549,14 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
       mbar_wait(bar_acc_full, 0);
       tc_fence_after();
     }
-    // half 0 writes dK (scaled), half 1 writes dV
-    const uint32_t tAcc = (half == 0 ? tDK : tDV) + lane_base;
-    const float mul = half == 0 ? scale : 1.f;
-    __nv_bfloat16* dst_base = (half == 0 ? dk : dv) + (static_cast<size_t>(srow) * n_kv_heads + hk) * D;
+    // parts 0,1 write the two column halves of dK (scaled), parts 2,3 those of dV
+    const bool is_dk = part < 2;
+    const int chalf = part & 1;
+    const uint32_t tAcc = (is_dk ? tDK : tDV) + lane_base + chalf * (D / 2);
+    const float mul = is_dk ? scale : 1.f;
+    __nv_bfloat16* dst_base = (is_dk ? dk : dv) + (static_cast<size_t>(srow) * n_kv_heads + hk) * D + chalf * (D / 2);
 #pragma unroll
-    for (int c = 0; c < D / 32; ++c) {
+    for (int c = 0; c < D / 64; ++c) {
       uint32_t v[32];
       if (n_iters > 0) {
         tmem_ld32(tAcc + c * 32, v);
