@@ -144,7 +144,7 @@ static int launch_bwd(const PlanDevice* pd, const void* dout, const void* q, con
   SAP_CUDA_CHECK(cudaGetLastError());
   }
   if (stages & 4) {
-  sap_bwd_dq_kernel<D><<<static_cast<unsigned>(pd->fwd.n_tiles) * Hq, kFwdThreads, DqSmem<D>::kTotal, stream>>>(
+  sap_bwd_dq_kernel<D><<<static_cast<unsigned>(pd->fwd.n_tiles) * Hq, kDqThreads, DqSmem<D>::kTotal, stream>>>(
       mq128, mdo128, mk64, mv64, pd->fwd.tiles, pd->fwd.segs, cu, plan->n_docs, lse, dsum,
       static_cast<__nv_bfloat16*>(dq), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
   g_launch_count.fetch_add(1);

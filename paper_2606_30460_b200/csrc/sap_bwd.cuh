@@ -74,230 +74,6 @@ __device__ unsigned long long g_sap_trace[128 * 64];
 #endif
 
 // ------------------------------------------------------------------------------------------------
-// dQ kernel.  One CTA = one 128-row Q tile x one q-head, two CTAs per SM (same recipe as the forward).
-// TMEM (256 columns): [0,64) S fp32 -> dS bf16 in [0,32); [64,128) dP fp32; [128,128+D) dQ fp32.
-// smem: Q, dO (128 x D), K double-buffered (64 x D), V (64 x D).
-// ------------------------------------------------------------------------------------------------
-template <int D>
-struct DqSmem {
-  static constexpr int kQBytes = kTile * D * 2;
-  static constexpr int kKBytes = kBwdN * D * 2;
-  static constexpr int kQBox = kTile * 128;   // 128 rows x 128 B
-  static constexpr int kKBox = kBwdN * 128;   // 64 rows x 128 B
-  static constexpr int kBoxes = D / 64;
-  static constexpr int kOffQ = 0, kOffDO = kQBytes, kOffK = 2 * kQBytes, kOffV = 2 * kQBytes + 2 * kKBytes;
-  static constexpr int kBarOffset = kOffV + kKBytes;
-  static constexpr int kTotal = kBarOffset + 256;  // dynamic smem base is required to be 1024 B aligned
-};
-
-template <int D>
-__global__ void __launch_bounds__(kFwdThreads, 2)
-sap_bwd_dq_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapDO,
-                  const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
-                  const TileDesc* __restrict__ tiles, const SegDesc* __restrict__ segs,
-                  const int32_t* __restrict__ cu, int n_docs, const float* __restrict__ lse,
-                  const float* __restrict__ dsum, __nv_bfloat16* __restrict__ dq, int n_tokens, int n_q_heads,
-                  int n_kv_heads, float scale, float scale_log2) {
-  using L = DqSmem<D>;
-  extern __shared__ __align__(1024) uint8_t smem_raw[];
-  uint8_t* smem = smem_raw;
-  if (smem_u32(smem) & 1023u) __trap();
-  const uint32_t sQ = smem_u32(smem) + L::kOffQ, sDO = smem_u32(smem) + L::kOffDO, sK = smem_u32(smem) + L::kOffK,
-                 sV = smem_u32(smem) + L::kOffV;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L::kBarOffset);
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kBarOffset + 128);
-  const uint32_t bar_q_full = smem_u32(bars + 0), bar_k_full = smem_u32(bars + 1) /* +1: stage 1 */,
-                 bar_k_empty = smem_u32(bars + 3) /* +1 */, bar_v_full = smem_u32(bars + 5),
-                 bar_v_empty = smem_u32(bars + 6), bar_s_full = smem_u32(bars + 7), bar_ds_full = smem_u32(bars + 8) /* +1 */,
-                 bar_dq_full = smem_u32(bars + 10);
-
-  // logical warp id: the service warps (0-3: TMA, tcgen05 issuer, ...) are the physically LAST four warps, because the
-  // SM's warp arbiter favours high warp ids and the single issuing threads must never starve; +4 keeps warp % 4
-  // (the TMEM lane quarter) and the warpgroup split of setmaxnreg intact
-  const int warp = ((threadIdx.x >> 5) + 4) & 7, lane = threadIdx.x & 31;
-  const int tile_idx = blockIdx.x / n_q_heads, h = blockIdx.x % n_q_heads;
-  const int hk = h / (n_q_heads / n_kv_heads);
-  const TileDesc td = tiles[tile_idx];
-
-  if (threadIdx.x == 0) {
-    mbar_init(bar_q_full, 1);
-    mbar_init(bar_k_full, 1); mbar_init(bar_k_full + 8, 1);
-    mbar_init(bar_k_empty, 1); mbar_init(bar_k_empty + 8, 1);
-    mbar_init(bar_v_full, 1); mbar_init(bar_v_empty, 1); mbar_init(bar_s_full, 1);
-    mbar_init(bar_ds_full, 128); mbar_init(bar_ds_full + 8, 128); mbar_init(bar_dq_full, 1);
-    fence_mbar_init();
-    tma_prefetch_desc(&mapQ); tma_prefetch_desc(&mapDO); tma_prefetch_desc(&mapK); tma_prefetch_desc(&mapV);
-  }
-  if (warp == 1) { tmem_alloc(smem_u32(tmem_slot), 256); tmem_relinquish(); }
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = *tmem_slot;
-  const uint32_t tS = tmem, tDS = tmem, tDP = tmem + 64, tDQ = tmem + 128;
-
-  int n_iters = 0;
-  for (int s = td.seg_begin; s < td.seg_end; ++s) {
-    const int c_begin = segs[s].t_begin;  // 128-aligned; 64-wide tiles start there too
-    n_iters += (segs[s].t_end - c_begin + kBwdN - 1) / kBwdN;
-  }
-
-  if (warp == 0) {
-    reg_dealloc<56>();
-    if (n_iters > 0 && elect_one()) {
-      mbar_expect_tx(bar_q_full, 2 * L::kQBytes);
-#pragma unroll
-      for (int b = 0; b < L::kBoxes; ++b) {
-        tma_load_2d(sQ + b * L::kQBox, &mapQ, h * D + b * 64, td.row0, bar_q_full);
-        tma_load_2d(sDO + b * L::kQBox, &mapDO, h * D + b * 64, td.row0, bar_q_full);
-      }
-      int it = 0;
-      for (int s = td.seg_begin; s < td.seg_end; ++s) {
-        const int c_begin = segs[s].t_begin, c_end = segs[s].t_end;
-        for (int c0 = c_begin; c0 < c_end; c0 += kBwdN, ++it) {
-          const int st = it & 1;
-          mbar_wait(bar_k_empty + 8 * st, ((it >> 1) & 1) ^ 1);
-          mbar_expect_tx(bar_k_full + 8 * st, L::kKBytes);
-#pragma unroll
-          for (int b = 0; b < L::kBoxes; ++b)
-            tma_load_2d(sK + st * L::kKBytes + b * L::kKBox, &mapK, hk * D + b * 64, c0, bar_k_full + 8 * st);
-          mbar_wait(bar_v_empty, (it & 1) ^ 1);
-          mbar_expect_tx(bar_v_full, L::kKBytes);
-#pragma unroll
-          for (int b = 0; b < L::kBoxes; ++b) tma_load_2d(sV + b * L::kKBox, &mapV, hk * D + b * 64, c0, bar_v_full);
-        }
-      }
-    }
-  } else if (warp == 1) {
-    reg_dealloc<56>();
-    if (n_iters > 0) {
-      constexpr uint32_t idesc_s = make_idesc_bf16(128, kBwdN, 0, 0);  // S, dP [128x64]: K-major x K-major
-      constexpr uint32_t idesc_dq = make_idesc_bf16(128, D, 0, 1);     // dQ [128xD] = dS (TMEM) x K (MN-major)
-      mbar_wait(bar_q_full, 0);
-      for (int it = 0; it < n_iters; ++it) {
-        const int st = it & 1;
-        const uint32_t sKs = sK + st * L::kKBytes;
-        mbar_wait(bar_k_full + 8 * st, (it >> 1) & 1);
-        mbar_wait(bar_v_full, it & 1);
-        tc_fence_after();
-        if (elect_one()) {
-#pragma unroll
-          for (int k = 0; k < D / 16; ++k) {
-            const uint32_t offq = (k / 4) * L::kQBox + (k % 4) * 32, offk = (k / 4) * L::kKBox + (k % 4) * 32;
-            umma_ss(tS, make_smem_desc(sQ + offq, 16, 1024), make_smem_desc(sKs + offk, 16, 1024), idesc_s, k > 0);
-          }
-#pragma unroll
-          for (int k = 0; k < D / 16; ++k) {
-            const uint32_t offq = (k / 4) * L::kQBox + (k % 4) * 32, offk = (k / 4) * L::kKBox + (k % 4) * 32;
-            umma_ss(tDP, make_smem_desc(sDO + offq, 16, 1024), make_smem_desc(sV + offk, 16, 1024), idesc_s, k > 0);
-          }
-          umma_commit(bar_v_empty);
-          umma_commit(bar_s_full);
-        }
-        __syncwarp();
-#pragma unroll
-        for (int half = 0; half < 2; ++half) {  // dQ starts as soon as the first 32 keys of dS are in TMEM
-          mbar_wait(bar_ds_full + 8 * half, it & 1);
-          tc_fence_after();
-          if (elect_one()) {
-#pragma unroll
-            for (int k = half * 2; k < half * 2 + 2; ++k)
-              umma_ts(tDQ, tDS + k * 8, make_smem_desc(sKs + k * 2048, L::kKBox, 1024), idesc_dq, (it > 0 || k > 0) ? 1u : 0u);
-            if (half == 1) {
-              umma_commit(bar_k_empty + 8 * st);
-              if (it == n_iters - 1) umma_commit(bar_dq_full);
-            }
-          }
-          __syncwarp();
-        }
-      }
-    }
-  } else if (warp < 4) {
-    reg_dealloc<56>();
-  } else {
-    reg_alloc<200>();
-    const int r = (warp - 4) * 32 + lane;
-    const int t = td.row0 + r;
-    const bool valid = r < td.rows;
-    const uint32_t lane_base = static_cast<uint32_t>((warp - 4) * 32) << 16;
-    const int32_t doc_lo = valid ? doc_start_of(cu, n_docs, t) : 0;
-    const float lse2 = valid ? lse[static_cast<size_t>(h) * n_tokens + t] * kLog2e : CUDART_INF_F;
-    const float dsum_t = valid ? dsum[static_cast<size_t>(h) * n_tokens + t] : 0.f;
-    int it = 0;
-    for (int s = td.seg_begin; s < td.seg_end; ++s) {
-      const SegDesc sd = segs[s];
-      int lo = max(doc_lo, sd.kv_lo), hi = min(t + 1, sd.kv_hi);
-      if (!valid || t < sd.q_lo || t >= sd.q_hi) { lo = 0; hi = 0; }
-      for (int c0 = sd.t_begin; c0 < sd.t_end; c0 += kBwdN, ++it) {
-        mbar_wait(bar_s_full, it & 1);
-        tc_fence_after();
-        const bool need_mask = __any_sync(0xffffffffu, (c0 < lo) || (c0 + kBwdN > hi));
-        uint32_t sv[64], dp[64];
-#pragma unroll
-        for (int c = 0; c < 2; ++c) {
-          tmem_ld32(tS + lane_base + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[c * 32]));
-          tmem_ld32(tDP + lane_base + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&dp[c * 32]));
-        }
-        tmem_wait_ld();
-        if (need_mask) {  // boundary tiles only: masked scores become -inf => P = 0 => dS = 0
-#pragma unroll
-          for (int i = 0; i < 64; ++i) {
-            const int col = c0 + i;
-            if (!(col >= lo && col < hi)) sv[i] = 0xff800000u;
-          }
-        }
-#pragma unroll
-        for (int c = 0; c < 2; ++c) {
-          uint32_t pk[16];
-#pragma unroll
-          for (int i = 0; i < 32; i += 2) {
-            const float p0 = ex2_approx(fmaf(__uint_as_float(sv[c * 32 + i]), scale_log2, -lse2));
-            const float p1 = ex2_approx(fmaf(__uint_as_float(sv[c * 32 + i + 1]), scale_log2, -lse2));
-            pk[i >> 1] = pack_bf16x2(p0 * (__uint_as_float(dp[c * 32 + i]) - dsum_t),
-                                     p1 * (__uint_as_float(dp[c * 32 + i + 1]) - dsum_t));
-          }
-          tmem_st16(tDS + lane_base + c * 16, pk);
-          tmem_wait_st();
-          tc_fence_before();
-          mbar_arrive(bar_ds_full + 8 * c);
-        }
-      }
-    }
-    if (n_iters > 0) {
-      mbar_wait(bar_dq_full, 0);
-      tc_fence_after();
-    }
-    const size_t row_off = (static_cast<size_t>(t) * n_q_heads + h) * D;
-#pragma unroll
-    for (int c = 0; c < D / 32; ++c) {
-      uint32_t v[32];
-      if (n_iters > 0) {
-        tmem_ld32(tDQ + lane_base + c * 32, v);
-        tmem_wait_ld();
-      } else {
-#pragma unroll
-        for (int i = 0; i < 32; ++i) v[i] = 0u;
-      }
-      if (valid) {
-        uint4* dst = reinterpret_cast<uint4*>(dq + row_off + c * 32);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          uint4 w;
-          w.x = pack_bf16x2(__uint_as_float(v[8 * i + 0]) * scale, __uint_as_float(v[8 * i + 1]) * scale);
-          w.y = pack_bf16x2(__uint_as_float(v[8 * i + 2]) * scale, __uint_as_float(v[8 * i + 3]) * scale);
-          w.z = pack_bf16x2(__uint_as_float(v[8 * i + 4]) * scale, __uint_as_float(v[8 * i + 5]) * scale);
-          w.w = pack_bf16x2(__uint_as_float(v[8 * i + 6]) * scale, __uint_as_float(v[8 * i + 7]) * scale);
-          dst[i] = w;
-        }
-      }
-    }
-  }
-
-  tc_fence_before();
-  __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem, 256);
-}
-
-// ------------------------------------------------------------------------------------------------
 // dK/dV kernel.  One CTA = one 128-row K/V tile x one kv-head, one CTA per SM, 384 threads:
 //   warp 0 TMA producer, warp 1 tcgen05 issuer, warp 2 LSE/D loader, warps 4-11 compute
 //   (warp w: TMEM lane quarter w%4 = key rows, column half (w-4)/4 of the 64 streamed q rows).
@@ -586,3 +362,5 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
 }
 
 }  // namespace sap
+
+#include "sap_bwd_dq.cuh"
