@@ -147,11 +147,10 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     import paper_2606_30460_b200 as sap
-    from paper_2606_30460_b200.workloads import make_qkv, make_workload
+    from paper_2606_30460_b200 import shard
+    from paper_2606_30460_b200.workloads import make_qkv
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = shard.rank_world()
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
@@ -160,7 +159,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
 
     # each rank gets its own packed sequence (seed = rank): data-parallel units, no exchange
-    w = make_workload(args.config, seed=rank)
+    w = shard.rank_workload(args.config, rank)
     q, k, v, do = make_qkv(w, device=dev)
     plan = sap.sap_plan(w.cu_seqlens, w.n_chunks)
     plan.upload()
@@ -205,12 +204,7 @@ def run_ours(args):
     launches = sap.sap_launch_count() - launches0
     sync_all()
     clocks = sampler.stop() if rank == 0 else None
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    flops = torch.tensor([float(w.flops_fwd + w.flops_bwd)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(flops, op=dist.ReduceOp.SUM)
-    ms_max, flops_all = float(t.item()), float(flops.item())
+    ms_max, flops_all = shard.aggregate(ms, float(w.flops_fwd + w.flops_bwd), dev)   # MAX time, SUM work
     value = flops_all / (ms_max * 1e-3) / 1e12
 
     # ---- per-kernel times (separate passes; CUDA events on the launching stream), rank 0 reports
@@ -245,10 +239,8 @@ def run_ours(args):
     e_steps = max(2, min(args.steps, 5))
     ms_e2e = timed(e2e_step, e_steps)
     sync_all()
-    t2 = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t2, op=dist.ReduceOp.MAX)
-    e2e_value = flops_all / (float(t2.item()) * 1e-3) / 1e12
+    ms_e2e_max, _ = shard.aggregate(ms_e2e, 0.0, dev)
+    e2e_value = flops_all / (ms_e2e_max * 1e-3) / 1e12
     h2d = sum(x.numel() * x.element_size() for x in (hq, hk, hv, hdo))
     d2h = sum(x.numel() * x.element_size() for x in (r_out, r_lse, r_dq, r_dk, r_dv))
 
@@ -297,7 +289,7 @@ def run_ours(args):
             "bwd": {"ms": sum(per.values()), "tflops": w.flops_bwd / (sum(per.values()) * 1e-3) / 1e12},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "ms_per_step": float(t2.item())},
+                    "ms_per_step": ms_e2e_max},
             "gpu_launches": int(launches),
             "roofline": roofline,
             "kernels": kernels,

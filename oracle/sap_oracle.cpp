@@ -226,6 +226,9 @@ int sap_oracle_bwd_dq(const float* q, const float* k, const float* v, const floa
 //   dV_s =       sum_{h in group} sum_{t>=s, same doc} P_ts dO_t
 // Row statistics LSE_t, D_t are computed first (plain forward) for every row that some
 // listed column can see.                      out_dk, out_dv [n_cols,Hkv,d]
+// A row t whose dO_t is exactly zero in every head adds exactly zero to both sums
+// (dP_ts = 0 and D_t = 0 give dS_ts = 0; P_ts dO_t = 0), so such rows are skipped: no value
+// changes, and a test may probe all columns against a sparse set of live rows at full size.
 // ---------------------------------------------------------------------------------
 int sap_oracle_bwd_dkv(const float* q, const float* k, const float* v, const float* dout,
                        const int32_t* cu, int n_docs, int64_t N, int Hq, int Hkv, int d,
@@ -242,9 +245,16 @@ int sap_oracle_bwd_dkv(const float* q, const float* k, const float* v, const flo
     const int e = doc_of(cu, n_docs, s);
     first_col[e] = std::min(first_col[e], s);
   }
+  std::vector<char> live(N, 0);  // dO_t != 0 somewhere
+  for (int64_t t = 0; t < N; ++t) {
+    const float* row = dout + t * (int64_t)Hq * d;
+    for (int64_t c = 0; c < (int64_t)Hq * d; ++c)
+      if (row[c] != 0.0f) { live[t] = 1; break; }
+  }
   std::vector<int64_t> need;
   for (int e = 0; e < n_docs; ++e)
-    for (int64_t t = std::max<int64_t>(first_col[e], cu[e]); t < cu[e + 1]; ++t) need.push_back(t);
+    for (int64_t t = std::max<int64_t>(first_col[e], cu[e]); t < cu[e + 1]; ++t)
+      if (live[t]) need.push_back(t);
   std::vector<int64_t> slot(N, -1);
   for (size_t i = 0; i < need.size(); ++i) slot[need[i]] = (int64_t)i;
   std::vector<double> lse(need.size() * Hq), Dt(need.size() * Hq);
@@ -273,7 +283,8 @@ int sap_oracle_bwd_dkv(const float* q, const float* k, const float* v, const flo
       double* dk = out_dk + (i * Hkv + hk) * d;
       double* dv = out_dv + (i * Hkv + hk) * d;
       for (int c = 0; c < d; ++c) dk[c] = dv[c] = 0.0;
-      for (int64_t t = s; t < cu[e + 1]; ++t)
+      for (int64_t t = s; t < cu[e + 1]; ++t) {
+        if (!live[t]) continue;  // contributes exactly zero
         for (int h = hk * g; h < (hk + 1) * g; ++h) {
           const float* qt = q + (t * Hq + h) * d;
           const float* dot_ = dout + (t * Hq + h) * d;
@@ -285,6 +296,7 @@ int sap_oracle_bwd_dkv(const float* q, const float* k, const float* v, const flo
             dk[c] += scale * ds * (double)qt[c];
           }
         }
+      }
     }
   return 0;
 }

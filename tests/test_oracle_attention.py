@@ -272,3 +272,18 @@ def test_partial_rows_without_keys_are_empty():
     # rows 8..16 (second doc + tail) against keys 0..6 (first doc only): nothing visible
     o, lse = oracle.attn_partial(q, k, v, cu, 0.5, 8, 16, 0, 6)
     assert np.all(lse == -np.inf) and np.all(o == 0)
+
+
+def test_p1_sparse_dout_rows_match_brute_force():
+    # rows with dO = 0 are skipped by the oracle's dK/dV (they add exactly zero): same result as the full matrix form
+    cu, q, k, v, do = make([9, 14, 1, 8], 4, 2, 8, seed=3)
+    keep = np.zeros(len(q), dtype=bool); keep[[0, 5, 8, 9, 20, 22, 23, 31]] = True
+    do = np.where(keep[:, None, None], do, np.float32(0))
+    scale = 0.3
+    _, _, dQ, dK, dV = brute(q, k, v, cu, scale, do)
+    dk, dv = oracle.attn_bwd_dkv(q, k, v, do, cu, scale)
+    assert np.abs(dk - dK).max() < 1e-12 and np.abs(dv - dV).max() < 1e-12
+    cols = [0, 3, 9, 10, 22, 23, 24, 31]
+    dk2, dv2 = oracle.attn_bwd_dkv(q, k, v, do, cu, scale, cols=cols)
+    assert np.abs(dk2 - dK[cols]).max() < 1e-12 and np.abs(dv2 - dV[cols]).max() < 1e-12
+    assert np.abs(oracle.attn_bwd_dq(q, k, v, do, cu, scale) - dQ).max() < 1e-12
