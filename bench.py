@@ -193,6 +193,8 @@ def run_ours(args):
         torch.cuda.synchronize()
         return e0.elapsed_time(e1) / n  # ms per call
 
+    bwd_mask = 7 if args.bwd == "split" else -1   # -1 = library default (D pre-pass + fused main + dQ post pass)
+    sap.sap_debug_set_bwd_stages(bwd_mask)
     for _ in range(max(args.warmup, 3)):
         step()
     sync_all()
@@ -211,18 +213,21 @@ def run_ours(args):
     kn = max(3, min(args.steps, 10))
     t_fwd = timed(fwd, kn)
     per = {}
-    for name, mask in (("bwd_pre", 1), ("bwd_dkv", 2), ("bwd_dq", 4)):
+    stage_list = (("bwd_pre", 1), ("bwd_dkv", 2), ("bwd_dq", 4)) if args.bwd == "split" else \
+                 (("bwd_pre", 1), ("bwd_fused", 8), ("bwd_post", 16))
+    for name, mask in stage_list:
         sap.sap_debug_set_bwd_stages(mask)
         bwd(); torch.cuda.synchronize()
         per[name] = timed(bwd, kn)
-    sap.sap_debug_set_bwd_stages(7)
+    sap.sap_debug_set_bwd_stages(bwd_mask)
 
     # ---- end to end: host (pinned) buffers in, results back to host, copies inside the timed region
     if args.profile_only:
         if world > 1:
             dist.destroy_process_group()
         if rank == 0:
-            print(json.dumps({"profile_only": True, "ms_per_step": ms_max, "value": value, "fwd_ms": t_fwd, **per}))
+            print(json.dumps({"profile_only": True, "bwd": args.bwd, "ms_per_step": ms_max, "value": value, "fwd_ms": t_fwd, **per,
+                              "clocks": clocks}))
         return
     hq, hk, hv, hdo = (x.cpu().pin_memory() for x in (q, k, v, do))
     r_out, r_lse = torch.empty_like(hq).pin_memory(), torch.empty((Hq, N), dtype=torch.float32).pin_memory()
@@ -253,11 +258,16 @@ def run_ours(args):
         gemm = 2.0 * d * Hq * pairs
         kernels = {
             "sap_fwd_kernel": {"ms": t_fwd, "algorithmic_tflop": 2 * gemm / 1e12},
-            "sap_bwd_dkv_kernel": {"ms": per["bwd_dkv"], "algorithmic_tflop": 4 * gemm / 1e12},
-            "sap_bwd_dq_kernel": {"ms": per["bwd_dq"], "algorithmic_tflop": 1 * gemm / 1e12,
-                                  "executed_tflop": 3 * gemm / 1e12},
             "sap_bwd_pre_kernel": {"ms": per["bwd_pre"], "algorithmic_gbytes": (2 * N * Hq * d * 2 + N * Hq * 4) / 1e9},
         }
+        if args.bwd == "split":
+            kernels["sap_bwd_dkv_kernel"] = {"ms": per["bwd_dkv"], "algorithmic_tflop": 4 * gemm / 1e12}
+            kernels["sap_bwd_dq_kernel"] = {"ms": per["bwd_dq"], "algorithmic_tflop": 1 * gemm / 1e12,
+                                            "executed_tflop": 3 * gemm / 1e12}
+        else:
+            # fused main kernel: all 5 GEMMs of the backward; its time includes zeroing the fp32 dQ accumulator
+            kernels["sap_bwd_fused_kernel"] = {"ms": per["bwd_fused"], "algorithmic_tflop": 5 * gemm / 1e12}
+            kernels["sap_bwd_post_kernel"] = {"ms": per["bwd_post"], "algorithmic_gbytes": N * Hq * d * 6 / 1e9}
         for kk, vv in kernels.items():
             if "algorithmic_tflop" in vv:
                 vv["tflops"] = vv["algorithmic_tflop"] / (vv["ms"] * 1e-3)
@@ -280,7 +290,7 @@ def run_ours(args):
                        "n_chunks": w.n_chunks, "n_docs": len(w.doc_lens), "n_q_heads": Hq, "n_kv_heads": Hkv,
                        "head_dim": d, "cu_seqlens_sha256": w.sha256(), "useful_pairs": pairs,
                        "plan_items": plan.n_items, "l2": "inputs exceed L2 (Q alone is %.0f MiB)" % (q.numel() * 2 / 2**20),
-                       "per_rank": "independent sequence per rank (seed = rank)"},
+                       "per_rank": "independent sequence per rank (seed = rank)", "bwd": args.bwd},
             "tokens_per_s": N * world / (ms_max * 1e-3),
             "frac_of_bf16_peak": {"measured_burst": value / world / peaks["bf16_burst"],
                                   "measured_sustained": value / world / peaks["bf16_sustained"],
@@ -311,6 +321,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, help="1..5 = BASELINE.json configs[0..4]")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--bwd", default="fused", choices=["fused", "split"],
+                    help="backward form: fused 5-GEMM kernel (default) or the split dK/dV + dQ kernels (diagnostic)")
     ap.add_argument("--profile-only", action="store_true",
                     help="stop after the device-timed region and the per-kernel passes (for ncu runs)")
     args = ap.parse_args()

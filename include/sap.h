@@ -93,7 +93,8 @@ int sap_plan_upload(sap_plan_t* plan);
 /* ---- attention ------------------------------------------------------------------------------ */
 enum { SAP_PASS_FWD = 0, SAP_PASS_BWD = 1 };
 
-/* Bytes of caller-provided device workspace a pass needs (fwd: 0; bwd: D = rowsum(dO*O), fp32 [Hq,N]). */
+/* Bytes of caller-provided device workspace a pass needs (fwd: 0; bwd: D = rowsum(dO*O), fp32 [Hq,N], padded to
+ * 256 B, followed by the fp32 dQ accumulator [N,Hq,d] the fused backward kernel reduces into). */
 size_t sap_workspace_bytes(const sap_plan_t* plan, int n_q_heads, int n_kv_heads, int head_dim, int pass);
 
 /* Forward: for every row, attention over the visible keys, walking the row's
@@ -130,7 +131,8 @@ int sap_lse_merge(const float* o_a, const float* lse_a, const float* o_b, const 
  * dV = P^T dO; dK/dV are summed over the Hq/Hkv q-heads of a group.
  * dout,q,k,v,out,lse,cu_seqlens_dev: device, read (out/lse as written by sap_attn_fwd).
  * dq [N,Hq,d], dk,dv [N,Hkv,d]: device bf16, written (every element).  workspace: device, at least
- * sap_workspace_bytes(plan, ..., SAP_PASS_BWD) bytes. */
+ * sap_workspace_bytes(plan, ..., SAP_PASS_BWD) bytes.  dQ is reduced in fp32 with atomic adds, so its low
+ * bits may differ from run to run (any accumulation order is correct, A-14); dK, dV are deterministic. */
 int sap_attn_bwd(const void* dout, const void* q, const void* k, const void* v, const void* out,
                  const float* lse, const int32_t* cu_seqlens_dev, sap_plan_t* plan,
                  void* dq, void* dk, void* dv,
@@ -142,9 +144,12 @@ const char* sap_strerror(int status);
 int sap_last_cuda_error(void);      /* the cudaError_t / CUresult of the last SAP_ERR_CUDA on this thread */
 /* Number of kernels the library has launched in this process (all streams); for launch accounting. */
 int64_t sap_launch_count(void);
-/* Diagnostic: which kernels sap_attn_bwd launches, so each can be timed alone (bit 0 = D pre-pass,
- * bit 1 = dK/dV kernel, bit 2 = dQ kernel; default 7 = all).  Process-wide; returns the previous mask.
- * With a partial mask the skipped outputs are left untouched. */
+/* Diagnostic: which kernels sap_attn_bwd launches, so each can be timed alone and the two forms of the main
+ * pass compared.  Bits: 1 = D pre-pass, 8 = fused main kernel (dK, dV, fp32 dQ accumulator; 5 GEMMs per tile
+ * pair; zeroes the accumulator first), 16 = dQ post pass (bf16(scale * accumulator)); 2 = split dK/dV kernel,
+ * 4 = split dQ kernel (the deterministic, atomics-free form: 7 GEMMs per tile pair).  Default 1|8|16; a negative
+ * mask restores the default.  Process-wide; returns the previous mask.  With a partial mask the skipped outputs
+ * are left untouched. */
 int sap_debug_set_bwd_stages(int mask);
 
 #ifdef __cplusplus

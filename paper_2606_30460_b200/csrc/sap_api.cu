@@ -5,13 +5,19 @@
 #include "sap_host.h"
 #include "sap_fwd.cuh"
 #include "sap_bwd.cuh"
+#include "sap_bwd_fused.cuh"
 #include "sap_merge.cuh"
 
 namespace sap {
 
+// sap_debug_set_bwd_stages bits: 1 D pre-pass | 2 split dK/dV kernel | 4 split dQ kernel | 8 fused main kernel
+// (+ zeroing of its fp32 dQ accumulator) | 16 dQ post pass.  Default: pre + fused + post.
+constexpr int kBwdDefaultStages = 1 | 8 | 16;
+static inline size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
+
 thread_local int g_last_cuda_error = 0;
 std::atomic<int64_t> g_launch_count{0};
-std::atomic<int> g_bwd_stages{7};
+std::atomic<int> g_bwd_stages{kBwdDefaultStages};
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -106,7 +112,7 @@ static int launch_fwd(const DevProgram& prog, const void* q, const void* k, cons
 template <int D>
 static int launch_bwd(const PlanDevice* pd, const void* dout, const void* q, const void* k, const void* v,
                       const void* out, const float* lse, const int32_t* cu, const sap_plan_t* plan, void* dq, void* dk,
-                      void* dv, int Hq, int Hkv, float scale, float* dsum, cudaStream_t stream) {
+                      void* dv, int Hq, int Hkv, float scale, float* dsum, float* dq_acc, cudaStream_t stream) {
   const int64_t N = plan->n_tokens;
   int rc;
   const int stages = g_bwd_stages.load();
@@ -133,7 +139,26 @@ static int launch_bwd(const PlanDevice* pd, const void* dout, const void* q, con
   if (!attr_set) {
     SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_dq_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, DqSmem<D>::kTotal));
     SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_dkv_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, DkvSmem<D>::kTotal));
+    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_fused_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FusedSmem<D>::kTotal));
     attr_set = true;
+  }
+  // a6 fused: dK, dV and the fp32 dQ accumulator in one pass (5 GEMMs per tile pair)
+  if (stages & 8) {
+    SAP_CUDA_CHECK(cudaMemsetAsync(dq_acc, 0, static_cast<size_t>(N) * Hq * D * sizeof(float), stream));
+    sap_bwd_fused_kernel<D><<<static_cast<unsigned>(pd->kv.n_tiles) * Hkv, kFusedThreads, FusedSmem<D>::kTotal, stream>>>(
+        mq64, mdo64, mk128, mv128, pd->kv.tiles, pd->kv.segs, cu, plan->n_docs, lse, dsum, dq_acc,
+        static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
+    g_launch_count.fetch_add(1);
+    SAP_CUDA_CHECK(cudaGetLastError());
+  }
+  // a7: dq = bf16(scale * dq_acc)
+  if (stages & 16) {
+    const int64_t n8 = N * Hq * D / 8;
+    const int64_t want = (n8 + kPostThreads - 1) / kPostThreads;
+    const unsigned grid = static_cast<unsigned>(want < 148 * 16 ? want : 148 * 16);
+    sap_bwd_post_kernel<<<grid, kPostThreads, 0, stream>>>(dq_acc, static_cast<__nv_bfloat16*>(dq), n8, scale);
+    g_launch_count.fetch_add(1);
+    SAP_CUDA_CHECK(cudaGetLastError());
   }
   // a6 (dK/dV half first: it is the longer kernel)
   if (stages & 2) {
@@ -166,7 +191,7 @@ int sap_debug_read_trace(unsigned long long* host_out) {
   return (int)cudaMemcpyFromSymbol(host_out, g_sap_trace, sizeof(unsigned long long) * 128 * 64);
 }
 #endif
-int sap_debug_set_bwd_stages(int mask) { return g_bwd_stages.exchange(mask & 7); }
+int sap_debug_set_bwd_stages(int mask) { return g_bwd_stages.exchange(mask < 0 ? kBwdDefaultStages : (mask & 31)); }
 
 int sap_plan_upload(sap_plan_t* plan) {
   if (!plan) return SAP_ERR_INVALID_ARG;
@@ -196,9 +221,11 @@ void sap_plan_destroy(sap_plan_t* plan) {
 }
 
 size_t sap_workspace_bytes(const sap_plan_t* plan, int n_q_heads, int n_kv_heads, int head_dim, int pass) {
-  (void)n_kv_heads; (void)head_dim;
+  (void)n_kv_heads;
   if (!plan || pass != SAP_PASS_BWD) return 0;
-  return static_cast<size_t>(plan->n_tokens) * n_q_heads * sizeof(float);  // D = rowsum(dO * O), fp32 [Hq, N]
+  // D = rowsum(dO * O), fp32 [Hq, N]  |  dQ accumulator, fp32 [N, Hq, d]
+  return align256(static_cast<size_t>(plan->n_tokens) * n_q_heads * sizeof(float)) +
+         static_cast<size_t>(plan->n_tokens) * n_q_heads * head_dim * sizeof(float);
 }
 
 int sap_attn_fwd(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev, sap_plan_t* plan,
@@ -287,11 +314,14 @@ int sap_attn_bwd(const void* dout, const void* q, const void* k, const void* v, 
   if ((rc = sap_plan_upload(plan)) != SAP_OK) return rc;
   const PlanDevice* pd = static_cast<const PlanDevice*>(plan->dev_state);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  float* dsum = static_cast<float*>(workspace);
+  float* dq_acc = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) +
+                                           align256(static_cast<size_t>(plan->n_tokens) * n_q_heads * sizeof(float)));
   if (head_dim == 128)
     return launch_bwd<128>(pd, dout, q, k, v, out, lse, cu_seqlens_dev, plan, dq, dk, dv, n_q_heads, n_kv_heads,
-                           softmax_scale, static_cast<float*>(workspace), st);
+                           softmax_scale, dsum, dq_acc, st);
   return launch_bwd<64>(pd, dout, q, k, v, out, lse, cu_seqlens_dev, plan, dq, dk, dv, n_q_heads, n_kv_heads,
-                        softmax_scale, static_cast<float*>(workspace), st);
+                        softmax_scale, dsum, dq_acc, st);
 }
 
 }  // extern "C"
