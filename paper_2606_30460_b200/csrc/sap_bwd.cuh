@@ -122,7 +122,8 @@ sap_bwd_dkv_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
 
   // logical warp id: service warps (0-3) are the physically last four (see sap_fwd.cuh)
   const int warp = ((threadIdx.x >> 5) + 4) % (kDkvThreads / 32), lane = threadIdx.x & 31;
-  const int tile_idx = blockIdx.x / n_kv_heads, hk = blockIdx.x % n_kv_heads;
+  int tile_idx, hk;
+  kv_block_coords(n_kv_heads, tile_idx, hk);
   const int g = n_q_heads / n_kv_heads;
   const TileDesc td = tiles[tile_idx];
 

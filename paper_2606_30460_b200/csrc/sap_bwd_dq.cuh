@@ -53,7 +53,8 @@ sap_bwd_dq_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constan
 
   // logical warp id: service warps (0-3) are the physically last four (see sap_fwd.cuh)
   const int warp = ((threadIdx.x >> 5) + 4) % (kDqThreads / 32), lane = threadIdx.x & 31;
-  const int tile_idx = blockIdx.x / n_q_heads, h = blockIdx.x % n_q_heads;
+  int tile_idx, h;
+  q_block_coords(n_q_heads, n_kv_heads, tile_idx, h);
   const int hk = h / (n_q_heads / n_kv_heads);
   const TileDesc td = tiles[tile_idx];
 

@@ -42,6 +42,20 @@ __device__ __forceinline__ int32_t doc_start_of(const int32_t* __restrict__ cu, 
   return __ldg(cu + lo);
 }
 
+// Grid order: kv-head-major, tiles longest-first inside a head.  The CTAs that run side by side then work on the same
+// kv-head, whose K/V (and the Q / dO / dQ rows of its q-heads) fit in the 126 MB L2, instead of on all heads at once.
+__device__ __forceinline__ void q_block_coords(int n_q_heads, int n_kv_heads, int& tile_idx, int& h) {
+  const int g = n_q_heads / n_kv_heads, per_head = (gridDim.x / n_q_heads) * g;
+  const int hk = blockIdx.x / per_head, rem = blockIdx.x % per_head;
+  tile_idx = rem / g;
+  h = hk * g + rem % g;
+}
+__device__ __forceinline__ void kv_block_coords(int n_kv_heads, int& tile_idx, int& hk) {
+  const int n_tiles = gridDim.x / n_kv_heads;
+  hk = blockIdx.x / n_tiles;
+  tile_idx = blockIdx.x % n_tiles;
+}
+
 template <int D, bool PARTIAL>
 __global__ void __launch_bounds__(kFwdThreads, 2)
 sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
@@ -63,7 +77,8 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
   // SM's warp arbiter favours high warp ids and the single issuing threads must never starve; +4 keeps warp % 4
   // (the TMEM lane quarter) and the warpgroup split of setmaxnreg intact
   const int warp = ((threadIdx.x >> 5) + 4) & 7, lane = threadIdx.x & 31;
-  const int tile_idx = blockIdx.x / n_q_heads, h = blockIdx.x % n_q_heads;
+  int tile_idx, h;
+  q_block_coords(n_q_heads, n_kv_heads, tile_idx, h);
   const int hk = h / (n_q_heads / n_kv_heads);
   const TileDesc td = tiles[tile_idx];
 
