@@ -290,7 +290,8 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {w.name}", "n_tokens": N,
+            "config": {"workload": (f"BASELINE.json configs[{args.config - 1}]: {w.name}" if args.config <= 5 else
+                                    f"paper Table 2 shape (context, not a BASELINE config): {w.name}"), "n_tokens": N,
                        "n_chunks": w.n_chunks, "n_docs": len(w.doc_lens), "n_q_heads": Hq, "n_kv_heads": Hkv,
                        "head_dim": d, "cu_seqlens_sha256": w.sha256(), "useful_pairs": pairs,
                        "plan_items": plan.n_items, "l2": "inputs exceed L2 (Q alone is %.0f MiB)" % (q.numel() * 2 / 2**20),
@@ -323,7 +324,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=3, help="1..5 = BASELINE.json configs[0..4]")
+    ap.add_argument("--config", type=int, default=3, help="1..5 = BASELINE.json configs[0..4]; 8192..131072 = the paper's Table 2 shape at that length (context)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--bwd", default="fused", choices=["fused", "split"],
                     help="backward form: fused 5-GEMM kernel (default) or the split dK/dV + dQ kernels (diagnostic)")
