@@ -226,8 +226,14 @@ def run_ours(args):
         if world > 1:
             dist.destroy_process_group()
         if rank == 0:
-            print(json.dumps({"profile_only": True, "bwd": args.bwd, "ms_per_step": ms_max, "value": value, "fwd_ms": t_fwd, **per,
-                              "clocks": clocks}))
+            bwd_ms = sum(per.values())
+            print(json.dumps({"profile_only": True, "workload": w.name, "n_tokens": N, "n_docs": len(w.doc_lens),
+                              "useful_pairs": w.pairs, "plan_items": plan.n_items, "cu_seqlens_sha256": w.sha256(),
+                              "bwd": args.bwd, "ms_per_step": ms_max, "value": value,
+                              "frac_of_measured_burst_peak": value / world / load_peaks()["bf16_burst"],
+                              "tokens_per_s": N * world / (ms_max * 1e-3), "fwd_ms": t_fwd,
+                              "fwd_tflops": w.flops_fwd / (t_fwd * 1e-3) / 1e12, "bwd_ms": bwd_ms,
+                              "bwd_tflops": w.flops_bwd / (bwd_ms * 1e-3) / 1e12, **per, "clocks": clocks}))
         return
     hq, hk, hv, hdo = (x.cpu().pin_memory() for x in (q, k, v, do))
     r_out, r_lse = torch.empty_like(hq).pin_memory(), torch.empty((Hq, N), dtype=torch.float32).pin_memory()
