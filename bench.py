@@ -195,6 +195,7 @@ def run_ours(args):
 
     bwd_mask = 7 if args.bwd == "split" else -1   # -1 = library default (D pre-pass + fused main + dQ post pass)
     sap.sap_debug_set_bwd_stages(bwd_mask)
+    sap.sap_debug_set_fwd_form(1 if args.fwd == "single" else 0)
     for _ in range(max(args.warmup, 3)):
         step()
     sync_all()
@@ -332,6 +333,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, help="1..5 = BASELINE.json configs[0..4]; 8192..131072 = the paper's Table 2 shape at that length (context)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--fwd", default="pair", choices=["pair", "single"],
+                    help="forward kernel: two q-heads per CTA (default when Hq/Hkv is even) or one (diagnostic)")
     ap.add_argument("--bwd", default="fused", choices=["fused", "split"],
                     help="backward form: fused 5-GEMM kernel (default) or the split dK/dV + dQ kernels (diagnostic)")
     ap.add_argument("--profile-only", action="store_true",

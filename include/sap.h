@@ -144,6 +144,10 @@ const char* sap_strerror(int status);
 int sap_last_cuda_error(void);      /* the cudaError_t / CUresult of the last SAP_ERR_CUDA on this thread */
 /* Number of kernels the library has launched in this process (all streams); for launch accounting. */
 int64_t sap_launch_count(void);
+/* Diagnostic: which forward kernel sap_attn_fwd / sap_attn_fwd_partial launch.  0 (default): the pair kernel (two
+ * q-heads of one GQA group per CTA, sharing the K/V tiles) whenever Hq/Hkv is even, the one-head kernel otherwise;
+ * 1: always the one-head kernel.  Process-wide; returns the previous value. */
+int sap_debug_set_fwd_form(int form);
 /* Diagnostic: which kernels sap_attn_bwd launches, so each can be timed alone and the two forms of the main
  * pass compared.  Bits: 1 = D pre-pass, 8 = fused main kernel (dK, dV, fp32 dQ accumulator; 5 GEMMs per tile
  * pair; zeroes the accumulator first), 16 = dQ post pass (bf16(scale * accumulator)); 2 = split dK/dV kernel,

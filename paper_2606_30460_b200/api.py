@@ -205,3 +205,8 @@ def sap_launch_count() -> int:
 def sap_debug_set_bwd_stages(mask: int) -> int:
     """Diagnostic: select the kernels sap_attn_bwd launches (1 = D pre-pass, 2 = dK/dV, 4 = dQ)."""
     return int(_lib.lib().sap_debug_set_bwd_stages(int(mask)))
+
+
+def sap_debug_set_fwd_form(form: int) -> int:
+    """Diagnostic: 0 = pair forward kernel when Hq/Hkv is even (default), 1 = always the one-head kernel."""
+    return int(_lib.lib().sap_debug_set_fwd_form(int(form)))

@@ -4,6 +4,7 @@
 #include <cstring>
 #include "sap_host.h"
 #include "sap_fwd.cuh"
+#include "sap_fwd_pair.cuh"
 #include "sap_bwd.cuh"
 #include "sap_bwd_fused.cuh"
 #include "sap_merge.cuh"
@@ -18,6 +19,7 @@ static inline size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
 thread_local int g_last_cuda_error = 0;
 std::atomic<int64_t> g_launch_count{0};
 std::atomic<int> g_bwd_stages{kBwdDefaultStages};
+std::atomic<int> g_fwd_form{0};  // 0: pair kernel when Hq/Hkv is even, 1: always the one-head kernel (diagnostic)
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -95,10 +97,21 @@ static int launch_fwd(const DevProgram& prog, const void* q, const void* k, cons
   if ((rc = make_tile_map(&mk, k, plan->n_tokens, (int64_t)Hkv * D)) != SAP_OK) return rc;
   if ((rc = make_tile_map(&mv, v, plan->n_tokens, (int64_t)Hkv * D)) != SAP_OK) return rc;
   auto kern = sap_fwd_kernel<D, PARTIAL>;
+  auto kern_pair = sap_fwd_pair_kernel<D, PARTIAL>;
   static bool attr_set = false;
   if (!attr_set) {
     SAP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdSmem<D>::kTotal));
+    SAP_CUDA_CHECK(cudaFuncSetAttribute(kern_pair, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdPairSmem<D>::kTotal));
     attr_set = true;
+  }
+  if ((Hq / Hkv) % 2 == 0 && g_fwd_form.load() == 0) {  // two q-heads of a GQA group per CTA share the K/V stream
+    const unsigned grid = static_cast<unsigned>(prog.n_tiles) * (Hq / 2);
+    kern_pair<<<grid, kFwdPairThreads, FwdPairSmem<D>::kTotal, stream>>>(mq, mk, mv, prog.tiles, prog.segs, cu, plan->n_docs,
+                                                                      static_cast<__nv_bfloat16*>(out), out_f32, lse,
+                                                                      plan->n_tokens, Hq, Hkv, scale * kLog2e);
+    g_launch_count.fetch_add(1);
+    SAP_CUDA_CHECK(cudaGetLastError());
+    return SAP_OK;
   }
   const unsigned grid = static_cast<unsigned>(prog.n_tiles) * Hq;
   kern<<<grid, kFwdThreads, FwdSmem<D>::kTotal, stream>>>(mq, mk, mv, prog.tiles, prog.segs, cu, plan->n_docs,
@@ -191,6 +204,7 @@ int sap_debug_read_trace(unsigned long long* host_out) {
   return (int)cudaMemcpyFromSymbol(host_out, g_sap_trace, sizeof(unsigned long long) * 128 * 64);
 }
 #endif
+int sap_debug_set_fwd_form(int form) { return g_fwd_form.exchange(form ? 1 : 0); }
 int sap_debug_set_bwd_stages(int mask) { return g_bwd_stages.exchange(mask < 0 ? kBwdDefaultStages : (mask & 31)); }
 
 int sap_plan_upload(sap_plan_t* plan) {

@@ -66,12 +66,6 @@ __device__ __forceinline__ int32_t doc_end_of(const int32_t* __restrict__ cu, in
 
 constexpr int kBwdN = 64;  // streamed tile rows in both backward kernels
 
-#ifdef SAP_TRACE  // instrumented build only (never the shipped library): SM cycle stamps of one CTA
-__device__ unsigned long long g_sap_trace[128 * 64];
-#define SAP_STAMP(iter, slot) do { if (blockIdx.x == 0 && (iter) < 128) g_sap_trace[(iter) * 64 + (slot)] = clock64(); } while (0)
-#else
-#define SAP_STAMP(iter, slot) do { } while (0)
-#endif
 
 // ------------------------------------------------------------------------------------------------
 // dK/dV kernel.  One CTA = one 128-row K/V tile x one kv-head, one CTA per SM, 384 threads:

@@ -18,6 +18,13 @@
 
 namespace sap {
 
+#ifdef SAP_TRACE  // instrumented build only (never the shipped library): SM cycle stamps of one CTA
+__device__ unsigned long long g_sap_trace[128 * 64];
+#define SAP_STAMP(iter, slot) do { if (blockIdx.x == 0 && (iter) < 128) g_sap_trace[(iter) * 64 + (slot)] = clock64(); } while (0)
+#else
+#define SAP_STAMP(iter, slot) do { } while (0)
+#endif
+
 constexpr int kFwdThreads = 256;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;

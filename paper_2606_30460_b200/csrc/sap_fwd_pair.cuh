@@ -1,0 +1,304 @@
+// Forward kernel, pair form: one CTA = one 128-row Q tile x TWO q-heads of one GQA group, one CTA per SM.
+// (`computing` of PAPER.md Table 1 (:85-98) with the "copy and rescale" merge (:239) fused, as in sap_fwd.cuh.)
+//
+// The two heads attend the same rows to the same keys, so they walk the same segments and share every K / V tile
+// in shared memory (one TMA fill per two score tiles).  Two softmax warpgroups (A, B: one thread per row) alternate
+// on the MUFU pipe while the tensor pipe runs the other head's GEMMs:
+//     tensor pipe:  ... PV_A(i)  S_A(i+1)  PV_B(i)  S_B(i+1)  PV_A(i+1) ...
+//     warpgroup A:      softmax_A(i+1) ----------------->
+//     warpgroup B:                          softmax_B(i+1) ----------------->
+// Used when Hq/Hkv is even; sap_fwd_kernel (one head per CTA, two CTAs per SM) serves the other shapes.
+//
+// Roles (384 threads): warpgroups A and B = softmax / correction / epilogue; service warpgroup = TMA producer
+// (one elected thread) and tcgen05 issuer (one elected thread).
+// TMEM (512 columns): [0,128) S_A -> P_A | [128,256) S_B -> P_B | [256,256+D) O_A | [384,384+D) O_B.
+#pragma once
+#include "sap_fwd.cuh"
+
+namespace sap {
+
+#define FWD_STAMP(iter, slot) SAP_STAMP(iter, slot)
+
+constexpr int kFwdPairThreads = 384;
+constexpr int kFwdPairStages = 2;  // K and V rings
+
+template <int D>
+struct FwdPairSmem {
+  static constexpr int kTileBytes = kTile * D * 2;
+  static constexpr int kBoxBytes = kTile * 128;
+  static constexpr int kBoxes = D / 64;
+  static constexpr int kOffQ = 0;                                   // Q_A, Q_B
+  static constexpr int kOffK = 2 * kTileBytes;                      // K ring
+  static constexpr int kOffV = kOffK + kFwdPairStages * kTileBytes; // V ring
+  static constexpr int kBarOffset = kOffV + kFwdPairStages * kTileBytes;
+  static constexpr int kTotal = kBarOffset + 256;
+};
+
+template <int D, bool PARTIAL>
+__global__ void __launch_bounds__(kFwdPairThreads, 1)
+sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
+                    const __grid_constant__ CUtensorMap mapV, const TileDesc* __restrict__ tiles,
+                    const SegDesc* __restrict__ segs, const int32_t* __restrict__ cu, int n_docs,
+                    __nv_bfloat16* __restrict__ out, float* __restrict__ out_f32, float* __restrict__ lse,
+                    int n_tokens, int n_q_heads, int n_kv_heads, float scale_log2) {
+  using L = FwdPairSmem<D>;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* smem = smem_raw;
+  if (smem_u32(smem) & 1023u) __trap();
+  const uint32_t s0 = smem_u32(smem);
+  const uint32_t sQ = s0 + L::kOffQ, sK = s0 + L::kOffK, sV = s0 + L::kOffV;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L::kBarOffset);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kBarOffset + 240);
+  const uint32_t bar_q_full = smem_u32(bars + 0), bar_k_full = smem_u32(bars + 1), bar_k_empty = smem_u32(bars + 3),
+                 bar_v_full = smem_u32(bars + 5), bar_v_empty = smem_u32(bars + 7),
+                 bar_s_full = smem_u32(bars + 9) /* [A, B] */, bar_p_full = smem_u32(bars + 11) /* [A0, A1, B0, B1] */,
+                 bar_o_full = smem_u32(bars + 15) /* [A, B] */;
+
+  // logical warp id: the service warpgroup (logical warps 0-3) is the physically last one (see sap_fwd.cuh)
+  const int warp = ((threadIdx.x >> 5) + 4) % (kFwdPairThreads / 32), lane = threadIdx.x & 31;
+  // grid order: kv-head-major, tiles longest-first inside a head, the g/2 head pairs of a tile adjacent
+  const int g = n_q_heads / n_kv_heads, pairs = g / 2;
+  const int per_head = (gridDim.x / (n_kv_heads * pairs)) * pairs;
+  const int hk = blockIdx.x / per_head, rem = blockIdx.x % per_head;
+  const int tile_idx = rem / pairs, h0 = hk * g + 2 * (rem % pairs);  // heads h0 (A) and h0 + 1 (B)
+  const TileDesc td = tiles[tile_idx];
+
+  if (threadIdx.x == 0) {
+    mbar_init(bar_q_full, 1);
+    for (int i = 0; i < kFwdPairStages; ++i) {
+      mbar_init(bar_k_full + 8 * i, 1); mbar_init(bar_k_empty + 8 * i, 1);
+      mbar_init(bar_v_full + 8 * i, 1); mbar_init(bar_v_empty + 8 * i, 1);
+    }
+    for (int i = 0; i < 2; ++i) { mbar_init(bar_s_full + 8 * i, 1); mbar_init(bar_o_full + 8 * i, 1); }
+    for (int i = 0; i < 4; ++i) mbar_init(bar_p_full + 8 * i, 128);
+    fence_mbar_init();
+    tma_prefetch_desc(&mapQ); tma_prefetch_desc(&mapK); tma_prefetch_desc(&mapV);
+  }
+  if (warp == 1) { tmem_alloc(smem_u32(tmem_slot), 512); tmem_relinquish(); }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_slot;
+
+  int n_iters = 0;
+  for (int s = td.seg_begin; s < td.seg_end; ++s) n_iters += (segs[s].t_end - segs[s].t_begin + kTile - 1) / kTile;
+
+  if (warp < 4) {
+    reg_dealloc<72>();
+    if (warp == 0) {
+      // ---------------------------------------------------------------- TMA producer
+      if (n_iters > 0 && elect_one()) {
+        mbar_expect_tx(bar_q_full, 2 * L::kTileBytes);
+#pragma unroll
+        for (int x = 0; x < 2; ++x)
+#pragma unroll
+          for (int b = 0; b < L::kBoxes; ++b)
+            tma_load_2d(sQ + x * L::kTileBytes + b * L::kBoxBytes, &mapQ, (h0 + x) * D + b * 64, td.row0, bar_q_full);
+        int st = 0, ph = 1;  // empty barriers: the first pass over the rings must not block
+        for (int s = td.seg_begin; s < td.seg_end; ++s) {
+          const int c_begin = segs[s].t_begin, c_end = segs[s].t_end;
+          for (int c0 = c_begin; c0 < c_end; c0 += kTile) {
+            mbar_wait(bar_k_empty + 8 * st, ph);
+            mbar_expect_tx(bar_k_full + 8 * st, L::kTileBytes);
+#pragma unroll
+            for (int b = 0; b < L::kBoxes; ++b)
+              tma_load_2d(sK + st * L::kTileBytes + b * L::kBoxBytes, &mapK, hk * D + b * 64, c0, bar_k_full + 8 * st);
+            mbar_wait(bar_v_empty + 8 * st, ph);
+            mbar_expect_tx(bar_v_full + 8 * st, L::kTileBytes);
+#pragma unroll
+            for (int b = 0; b < L::kBoxes; ++b)
+              tma_load_2d(sV + st * L::kTileBytes + b * L::kBoxBytes, &mapV, hk * D + b * 64, c0, bar_v_full + 8 * st);
+            if (++st == kFwdPairStages) { st = 0; ph ^= 1; }
+          }
+        }
+      }
+    } else if (warp == 1) {
+      // ---------------------------------------------------------------- tcgen05 issuer (one elected thread)
+      if (n_iters > 0 && elect_one()) {
+        constexpr uint32_t idesc_s = make_idesc_bf16(128, 128, 0, 0);  // S[128x128] = Q (K-major) x K^T (K-major)
+        constexpr uint32_t idesc_o = make_idesc_bf16(128, D, 0, 1);    // O[128xD]  = P (TMEM)   x V (MN-major)
+        auto issue_s = [&](int x, int st) {   // S_x = Q_x K^T for the K tile in stage st
+#pragma unroll
+          for (int k = 0; k < D / 16; ++k) {
+            const uint32_t off = (k / 4) * L::kBoxBytes + (k % 4) * 32;
+            umma_ss(tmem + 128 * x, make_smem_desc(sQ + x * L::kTileBytes + off, 16, 1024),
+                    make_smem_desc(sK + st * L::kTileBytes + off, 16, 1024), idesc_s, k > 0);
+          }
+          umma_commit(bar_s_full + 8 * x);
+        };
+        auto issue_pv = [&](int x, int st, int it) {  // O_x += P_x V, in two halves of 64 keys
+#pragma unroll
+          for (int half = 0; half < 2; ++half) {
+            mbar_wait(bar_p_full + 8 * (2 * x + half), it & 1);
+            tc_fence_after();
+#pragma unroll
+            for (int k = half * 4; k < half * 4 + 4; ++k)  // 16 keys per MMA: 2 groups of 8 rows (SBO 1024 B)
+              umma_ts(tmem + 256 + 128 * x, tmem + 128 * x + k * 8,
+                      make_smem_desc(sV + st * L::kTileBytes + k * 2048, L::kBoxBytes, 1024), idesc_o,
+                      (it > 0 || k > 0) ? 1u : 0u);
+          }
+          if (it == n_iters - 1) umma_commit(bar_o_full + 8 * x);
+        };
+        mbar_wait(bar_q_full, 0);
+        mbar_wait(bar_k_full, 0);
+        tc_fence_after();
+        issue_s(0, 0);
+        issue_s(1, 0);
+        umma_commit(bar_k_empty);
+        int st = 0, ph = 0;  // stage / phase of iteration `it`
+        for (int it = 0; it < n_iters; ++it) {
+          const int st_n = (st + 1 == kFwdPairStages) ? 0 : st + 1, ph_n = (st_n == 0) ? ph ^ 1 : ph;
+          const bool more = it + 1 < n_iters;
+          FWD_STAMP(it, 0);
+          mbar_wait(bar_v_full + 8 * st, ph);
+          FWD_STAMP(it, 1);
+          issue_pv(0, st, it);
+          FWD_STAMP(it, 2);
+          if (more) {
+            mbar_wait(bar_k_full + 8 * st_n, ph_n);
+            tc_fence_after();
+            issue_s(0, st_n);   // S_A(it+1) runs while warpgroup B is still in softmax_B(it)
+          }
+          FWD_STAMP(it, 3);
+          issue_pv(1, st, it);
+          FWD_STAMP(it, 4);
+          umma_commit(bar_v_empty + 8 * st);
+          if (more) {
+            issue_s(1, st_n);
+            umma_commit(bar_k_empty + 8 * st_n);
+          }
+          st = st_n; ph = ph_n;
+        }
+      }
+    }
+  } else {
+    // ------------------------------------------------------------------ softmax / correction / epilogue (A or B)
+    reg_alloc<216>();  // 256 x 216 + 128 x 72 = the 384 x 168 register pool
+    const int x = (warp - 4) >> 2;  // 0: head h0 (A), 1: head h0 + 1 (B)
+    const int h = h0 + x;
+    const int r = (warp & 3) * 32 + lane;
+    const int t = td.row0 + r;
+    const bool valid = r < td.rows;
+    const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
+    const uint32_t tS = tmem + 128 * x, tP = tS, tO = tmem + 256 + 128 * x;
+    const uint32_t bar_s = bar_s_full + 8 * x, bar_p = bar_p_full + 16 * x, bar_o = bar_o_full + 8 * x;
+    const int32_t doc_lo = valid ? doc_start_of(cu, n_docs, t) : 0;
+    float m_used = -CUDART_INF_F;  // reference max (log2 domain) the running sum and O are scaled by
+    float l_run = 0.f;
+    int it = 0;
+    for (int s = td.seg_begin; s < td.seg_end; ++s) {
+      const SegDesc sd = segs[s];
+      int lo = max(doc_lo, sd.kv_lo), hi = min(t + 1, sd.kv_hi);  // visible keys of this row: [lo, hi)
+      if (!valid || t < sd.q_lo || t >= sd.q_hi) { lo = 0; hi = 0; }
+      for (int c0 = sd.t_begin; c0 < sd.t_end; c0 += kTile, ++it) {
+        mbar_wait(bar_s, it & 1);
+        tc_fence_after();
+        if ((warp & 3) == 0 && lane == 0) FWD_STAMP(it, 16 + 8 * x);
+        const bool need_mask = __any_sync(0xffffffffu, (c0 < lo) || (c0 + kTile > hi));
+        uint32_t sv[128];  // the whole S row of this thread
+#pragma unroll
+        for (int c = 0; c < 4; ++c) tmem_ld32(tS + lane_base + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[c * 32]));
+        tmem_wait_ld();
+        if (need_mask) {  // boundary tiles only (document start, diagonal, item edge)
+#pragma unroll
+          for (int i = 0; i < 128; ++i) {
+            const int col = c0 + i;
+            if (!(col >= lo && col < hi)) sv[i] = 0xff800000u;  // -inf
+          }
+        }
+        float mx4[4] = {-CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F};
+#pragma unroll
+        for (int i = 0; i < 128; i += 4) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) mx4[e] = fmaxf(mx4[e], __uint_as_float(sv[i + e]));
+        }
+        const float m_new = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * scale_log2;
+        // lazy rescale: only when the max moved by more than 2^8 (or the row saw its first key)
+        const bool grow = m_new > m_used + kRescaleThreshold || (m_used == -CUDART_INF_F && m_new > -CUDART_INF_F);
+        if (__any_sync(0xffffffffu, grow)) {
+          const float f = grow ? ((m_used == -CUDART_INF_F) ? 0.f : ex2_approx(m_used - m_new)) : 1.f;
+          if (grow) { m_used = m_new; l_run *= f; }
+          if (it > 0) {  // S(it) complete => PV(it-1) complete (tensor pipe order): O may be rewritten
+#pragma unroll
+            for (int c = 0; c < D / 32; ++c) {
+              uint32_t v[32];
+              tmem_ld32(tO + lane_base + c * 32, v);
+              tmem_wait_ld();
+#pragma unroll
+              for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(__uint_as_float(v[i]) * f);
+              tmem_st32(tO + lane_base + c * 32, v);
+            }
+          }
+        }
+        const float neg_m = (m_used == -CUDART_INF_F) ? 0.f : -m_used;
+        float ls4[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+#pragma unroll
+          for (int c = half * 2; c < half * 2 + 2; ++c) {
+            uint32_t pk[16];
+#pragma unroll
+            for (int i = 0; i < 32; i += 2) {
+              const float p0 = ex2_approx(fmaf(__uint_as_float(sv[c * 32 + i]), scale_log2, neg_m));
+              const float p1 = ex2_approx(fmaf(__uint_as_float(sv[c * 32 + i + 1]), scale_log2, neg_m));
+              ls4[(i >> 1) & 3] += p0 + p1;
+              pk[i >> 1] = pack_bf16x2(p0, p1);
+            }
+            tmem_st16(tP + lane_base + c * 16, pk);
+          }
+          tmem_wait_st();
+          tc_fence_before();
+          mbar_arrive(bar_p + 8 * half);
+          if ((warp & 3) == 0 && lane == 0) FWD_STAMP(it, 17 + 8 * x + half);
+        }
+        l_run += (ls4[0] + ls4[1]) + (ls4[2] + ls4[3]);
+      }
+    }
+    // ---- epilogue: O / l -> global, LSE (natural log)
+    if (n_iters > 0) {
+      mbar_wait(bar_o, 0);
+      tc_fence_after();
+    }
+    const float inv_l = l_run > 0.f ? 1.f / l_run : 0.f;
+    const size_t row_off = (static_cast<size_t>(t) * n_q_heads + h) * D;
+#pragma unroll
+    for (int c = 0; c < D / 32; ++c) {
+      uint32_t v[32];
+      if (n_iters > 0) {
+        tmem_ld32(tO + lane_base + c * 32, v);
+        tmem_wait_ld();
+      } else {
+#pragma unroll
+        for (int i = 0; i < 32; ++i) v[i] = 0u;
+      }
+      if (valid) {
+        if (PARTIAL) {
+          float4* dst = reinterpret_cast<float4*>(out_f32 + row_off + c * 32);
+#pragma unroll
+          for (int i = 0; i < 8; ++i)
+            dst[i] = make_float4(__uint_as_float(v[4 * i]) * inv_l, __uint_as_float(v[4 * i + 1]) * inv_l,
+                                 __uint_as_float(v[4 * i + 2]) * inv_l, __uint_as_float(v[4 * i + 3]) * inv_l);
+        } else {
+          uint4* dst = reinterpret_cast<uint4*>(out + row_off + c * 32);
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            uint4 w;
+            w.x = pack_bf16x2(__uint_as_float(v[8 * i + 0]) * inv_l, __uint_as_float(v[8 * i + 1]) * inv_l);
+            w.y = pack_bf16x2(__uint_as_float(v[8 * i + 2]) * inv_l, __uint_as_float(v[8 * i + 3]) * inv_l);
+            w.z = pack_bf16x2(__uint_as_float(v[8 * i + 4]) * inv_l, __uint_as_float(v[8 * i + 5]) * inv_l);
+            w.w = pack_bf16x2(__uint_as_float(v[8 * i + 6]) * inv_l, __uint_as_float(v[8 * i + 7]) * inv_l);
+            dst[i] = w;
+          }
+        }
+      }
+    }
+    if (valid)
+      lse[static_cast<size_t>(h) * n_tokens + t] = l_run > 0.f ? (m_used + log2f(l_run)) * kLn2 : -CUDART_INF_F;
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem, 512);
+}
+
+}  // namespace sap
