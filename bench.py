@@ -284,14 +284,14 @@ def run_ours(args):
                 vv["frac_of_hbm"] = vv["gbs"] / peaks["hbm"]
         dom = max((kk for kk in kernels if "tflops" in kernels[kk]), key=lambda kk: kernels[kk]["ms"])
         # DRAM bytes per launch of the dominant kernel from the one `ncu --set full` capture of this workload
-        # (profiles/r1b_ncu.md: dram__bytes_read.sum + dram__bytes_write.sum); no capture for other configurations
-        traffic = 13.366827e9 + 7.927147e9 if (dom == "sap_bwd_fused_kernel" and args.config == 3 and rank == 0) else None
+        # (profiles/r1c_ncu.md: dram__bytes_read.sum + dram__bytes_write.sum); no capture for other configurations
+        traffic = 13.172744e9 + 7.687649e9 if (dom == "sap_bwd_fused_kernel" and args.config == 3 and rank == 0) else None
         roofline = {"kernel": dom, "bound": "tensor", "achieved": kernels[dom]["tflops"],
                     "peak": peaks["bf16_sustained"], "unit": "TFLOP/s",
                     "frac": kernels[dom]["tflops"] / peaks["bf16_sustained"], "traffic": traffic,
                     "peak_source": peaks["source"] + ", sustained bf16 (kernel timed inside a long step)",
                     "ms_per_launch": kernels[dom]["ms"],
-                    "traffic_source": "profiles/r1b_ncu.md (ncu --set full, one launch)" if traffic else None}
+                    "traffic_source": "profiles/r1c_ncu.md (ncu --set full, one launch)" if traffic else None}
         cdt, cfl, cthreads, cdesc = time_oracle_bounded(15.0)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

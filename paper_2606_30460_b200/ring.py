@@ -1,0 +1,110 @@
+"""SURVEY 8(f) NEXT-1 (host side): the forward pass with REAL ranks, one sequence chunk per rank.
+
+The paper's execute side (Table 1 :85-98): rank i owns Q_i, K_i, V_i (n = N/P rows, :59); K/V shards
+travel rank to rank, every kept chunk pair (i, j) is one `computing` instruction on rank i, and the partial
+results are merged "in an online manner" (:59).  Which shards travel is decided by the plan, not by the ring: a
+rank sends its K/V shard only to the ranks whose plan has a non-SKIP item against it (the "trim redundant
+communication" of :106), and each ring step is ONE batched isend/irecv that covers the whole group, which is what
+lets NCCL coalesce it (:124).  Step s+1's transfers are posted before step s is computed (:120-122).
+
+On B200 nodes every peer is one NVSwitch hop away, so the paper's NVLink / InfiniBand placement (:144) has no
+counterpart here: the schedule is the plan's ring order and nothing else.
+
+This module is the exchange schedule plus argument marshalling.  The arithmetic is behind two callables:
+`partial_fn(item_index, k_shard, v_shard) -> (o [n,Hq,d] fp32, lse [Hq,n] fp32)` for this rank's rows and
+`merge_fn(o_a, lse_a, o_b, lse_b) -> (o, lse)`.  `cuda_fns()` builds them from the C-ABI kernels
+(`sap_attn_fwd_partial`, `sap_lse_merge`); the CPU tests (gloo, world_size 2 and 4) inject the oracle's.  It has
+not run on more than one GPU (this build has one): correct by construction, covered on CPU.
+"""
+from __future__ import annotations
+
+from typing import Callable, List, Optional, Tuple
+
+from .api import Plan, SAP_MASK_SKIP
+
+
+def step_peers(plan: Plan, rank: int, step: int) -> Tuple[Optional[int], Optional[int]]:
+    """(dst, src) of ring step `step` >= 1 for `rank`: dst = rank + step gets my K/V shard iff its plan has a
+    non-SKIP item against chunk `rank`; src = rank - step sends me its shard iff my plan has one against it."""
+    P = plan.n_chunks
+    km = plan.kind_map
+    dst = rank + step if rank + step < P and km[rank + step, rank] != SAP_MASK_SKIP else None
+    src = rank - step if rank - step >= 0 and km[rank, rank - step] != SAP_MASK_SKIP else None
+    return dst, src
+
+
+def schedule(plan: Plan) -> List[List[Tuple[int, int]]]:
+    """All (src, dst) transfers per ring step, for the whole group (the same list on every rank)."""
+    P = plan.n_chunks
+    out = []
+    for step in range(1, P):
+        out.append([(r, r + step) for r in range(P - step) if plan.kind_map[r + step, r] != SAP_MASK_SKIP])
+    return out
+
+
+def sap_ring_fwd(kv_shard, plan: Plan, rank: int, partial_fn: Callable, merge_fn: Callable, group=None):
+    """Forward of chunk `rank`.  kv_shard: this rank's stacked K/V shard [2, n, Hkv, d] (any device / dtype
+    torch.distributed can send).  Returns the merged (o, lse) of this rank's rows."""
+    import torch
+    import torch.distributed as dist
+
+    P = plan.n_chunks
+    assert dist.get_world_size(group) == P, "one rank per sequence chunk"
+    items = plan.items
+    co = plan.chunk_offsets
+    my_items = {int(items[x, 1]): x for x in range(int(co[rank]), int(co[rank + 1]))}   # kv_chunk -> item index
+
+    def post(step):
+        """One batched isend/irecv for ring step `step`; returns (requests, receive buffer or None)."""
+        dst, src = step_peers(plan, rank, step)
+        ops, buf = [], None
+        if dst is not None:
+            ops.append(dist.P2POp(dist.isend, kv_shard, dst, group))
+        if src is not None:
+            buf = torch.empty_like(kv_shard)
+            ops.append(dist.P2POp(dist.irecv, buf, src, group))
+        return (dist.batch_isend_irecv(ops) if ops else []), buf
+
+    nxt = post(1) if P > 1 else ([], None)
+    o, lse = partial_fn(my_items[rank], kv_shard[0], kv_shard[1])            # step 0: the diagonal block
+    for step in range(1, P):
+        reqs, buf = nxt
+        nxt = post(step + 1) if step + 1 < P else ([], None)                 # next step's transfer overlaps this compute
+        for r in reqs:
+            r.wait()
+        j = rank - step
+        if buf is not None and j in my_items:
+            po, pl = partial_fn(my_items[j], buf[0], buf[1])
+            o, lse = merge_fn(o, lse, po, pl)
+    return o, lse
+
+
+def cuda_fns(q_shard, cu_seqlens_dev, plan: Plan, rank: int, softmax_scale: Optional[float] = None):
+    """(partial_fn, merge_fn) on the C-ABI kernels.  The kernels address tokens globally, so the rank keeps
+    full-length Q / K / V buffers of which only its own rows and the shard in flight are filled."""
+    import torch
+    from . import api
+
+    n, Hq, d = q_shard.shape
+    N = plan.n_tokens
+    dev = q_shard.device
+    lo, hi = rank * n, (rank + 1) * n
+    qg = torch.zeros((N, Hq, d), dtype=q_shard.dtype, device=dev)
+    qg[lo:hi] = q_shard
+    kg = vg = None
+
+    def partial_fn(item, k_shard, v_shard):
+        nonlocal kg, vg
+        if kg is None:
+            kg = torch.zeros((N,) + tuple(k_shard.shape[1:]), dtype=k_shard.dtype, device=dev)
+            vg = torch.zeros_like(kg)
+        j = int(plan.items[item, 1])
+        kg[j * n:(j + 1) * n] = k_shard
+        vg[j * n:(j + 1) * n] = v_shard
+        o, lse = api.sap_attn_fwd_partial(qg, kg, vg, cu_seqlens_dev, plan, item, item + 1, softmax_scale=softmax_scale)
+        return o[lo:hi].contiguous(), lse[:, lo:hi].contiguous()
+
+    def merge_fn(o_a, lse_a, o_b, lse_b):
+        return api.sap_lse_merge(o_a, lse_a, o_b, lse_b)
+
+    return partial_fn, merge_fn
