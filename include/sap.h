@@ -85,6 +85,24 @@ int64_t sap_plan_useful_pairs(const sap_plan_t* plan);          /* sum over docu
 /* Number of 128x128 score tiles the forward kernel issues per q-head (for issue-efficiency reports). */
 int64_t sap_plan_fwd_tiles(const sap_plan_t* plan);
 
+/* Compile Steps 2-3 (§3.2, :110-:118): which rank computes each item and at which stage, for P real ranks
+ * (one chunk per rank).  Host only; does not change what the single-GPU kernels do.
+ *   policy SAP_SCHED_RING     : item (i, j) on rank i at stage i - j (plain ring attention, :59).
+ *   policy SAP_SCHED_BALANCED : Step 2, per causal region (= document spanning chunks a..b, m = b-a+1): the diagonal
+ *       item stays on its rank at stage 0; a FULL item (i, j) stays on rank i at regional stage i-j when
+ *       i-j <= m/2, else it is computed by the idle early rank j (Q_i travels to the K/V, the partial travels back)
+ *       at regional stage m-(i-j) — the LightSeq / DistFlashAttn balancing the paper refers to (:116).
+ *       Step 3: a rank that sits in two regions is over-subscribed.  (a) While the busiest rank holds a FULL item
+ *       whose other end (rank i or j) has at least two items fewer, the item whose other end is least loaded moves
+ *       there.  (b) At most one item per rank per stage: a rank runs its items back to back in order of
+ *       (regional stage, q_chunk, kv_chunk); stage = position in that list (shards travel point to point, so any
+ *       order is legal).
+ * slots: host, [sap_plan_n_items], written in item order.  *n_stages = 1 + the largest stage.  The paper's Fig. 3 is
+ * missing from the extracted text; this is the reading recorded in DESIGN.md (R-5). */
+enum { SAP_SCHED_RING = 0, SAP_SCHED_BALANCED = 1 };
+typedef struct { int32_t rank, stage; } sap_slot_t;
+int sap_plan_schedule(const sap_plan_t* plan, int32_t policy, sap_slot_t* slots, int32_t* n_stages);
+
 /* Copy the compiled work lists to the current CUDA device (cudaMalloc + synchronous cudaMemcpy).
  * Called implicitly by the first sap_attn_* call that uses the plan; call it yourself to keep that
  * cost out of a timed region.  Idempotent, thread-safe. */

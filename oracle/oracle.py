@@ -189,3 +189,73 @@ def plan(cu_seqlens, n_chunks: int) -> Plan:
     if n < 0:
         raise ValueError({-1: "invalid argument", -2: "bad cu_seqlens", -3: "N not divisible by n_chunks"}[n])
     return Plan(items[:n].copy(), co, ko, ki[:n].copy(), km)
+
+
+def schedule(cu_seqlens, n_chunks: int, policy: int = 1):
+    """Compile Steps 2-3, written out step by step in plain Python from the reading in DESIGN.md
+    (R-5; the paper's Fig. 3 is missing).  Returns (slots int32 [n_items, 2] = (rank, stage), n_stages).
+
+    policy 0: plain ring (:59): item (i, j) on rank i at stage i - j.
+    policy 1: Step 2 per causal region (a document spanning chunks a..b, m = b - a + 1): diagonal items on their own
+    rank at stage 0; a FULL item (i, j) stays on rank i at regional stage i - j if i - j <= m // 2, else the early
+    rank j computes it at regional stage m - (i - j) (LightSeq-style balancing, :116).  Step 3: every rank runs at
+    most one item per stage: it runs its items back to back in order of (regional stage, i, j), stage = position
+    in that list (:118; shards travel point to point, so any order is legal); before that, Step 3a moves items off the busiest rank while
+    that lowers its load ("striving to balance the computation load across all SAP ranks globally", :118).
+    PARITY: pinned by validity (every item once, rank in {i, j}, one item per rank and stage), by the closed form
+    for one document (floor(P/2) + 1 stages, loads within 1) and by makespan bounds; the choice among valid
+    schedules is this reading's, not the paper's (figure missing) - "partially pinned".
+    """
+    pl = plan(cu_seqlens, n_chunks)
+    cu = [int(x) for x in cu_seqlens]
+    P = int(n_chunks)
+    n = cu[-1] // P
+    items = [tuple(int(v) for v in row) for row in pl.items]
+    slots = np.zeros((len(items), 2), dtype=np.int32)
+    if policy == 0:
+        for x, it in enumerate(items):
+            slots[x] = (it[0], it[0] - it[1])
+        return slots, (int(slots[:, 1].max()) + 1 if len(items) else 0)
+    regional = []
+    for x, it in enumerate(items):
+        i, j, doc_lo, kind = it[0], it[1], it[2], it[4]
+        if kind == DIAG:
+            slots[x, 0] = i
+            regional.append(0)
+            continue
+        a, b = cu[doc_lo] // n, (cu[doc_lo + 1] - 1) // n          # chunks the region's document spans
+        m, t = b - a + 1, i - j
+        if t <= m // 2:
+            slots[x, 0] = i
+            regional.append(t)
+        else:
+            slots[x, 0] = j
+            regional.append(m - t)
+    # Step 3a: global balance - while the busiest rank (lowest index on ties) holds a FULL item whose other end
+    # (the rank of its Q or of its K/V) has at least two items fewer, hand over the item whose other end is least
+    # loaded (lowest item index on ties); its regional stage becomes t on rank i, m - t on rank j.
+    load = [0] * P
+    for x in range(len(items)):
+        load[slots[x, 0]] += 1
+    while True:
+        R = max(range(P), key=lambda r: (load[r], -r))
+        cands = [x for x in range(len(items)) if slots[x, 0] == R and items[x][4] != DIAG]
+        if not cands:
+            break
+        other = lambda x: items[x][1] if R == items[x][0] else items[x][0]
+        x = min(cands, key=lambda x: (load[other(x)], x))
+        o = other(x)
+        if load[o] + 1 >= load[R]:
+            break
+        load[R] -= 1
+        load[o] += 1
+        slots[x, 0] = o
+        i, j, doc_lo = items[x][0], items[x][1], items[x][2]
+        m, t = (cu[doc_lo + 1] - 1) // n - cu[doc_lo] // n + 1, i - j
+        regional[x] = t if o == i else m - t
+    # Step 3b: stages
+    nxt = [0] * P
+    for x in sorted(range(len(items)), key=lambda x: (regional[x], items[x][0], items[x][1])):
+        slots[x, 1] = nxt[slots[x, 0]]          # a rank runs its items back to back in this order
+        nxt[slots[x, 0]] += 1
+    return slots, (int(slots[:, 1].max()) + 1 if len(items) else 0)

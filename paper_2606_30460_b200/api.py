@@ -11,6 +11,7 @@ from . import _lib
 
 SAP_MASK_SKIP, SAP_MASK_FULL, SAP_MASK_DIAG = 0, 1, 2
 SAP_PASS_FWD, SAP_PASS_BWD = 0, 1
+SAP_SCHED_RING, SAP_SCHED_BALANCED = 0, 1
 
 
 class SapError(RuntimeError):
@@ -101,6 +102,15 @@ class Plan:
     @property
     def fwd_tiles(self) -> int:
         return int(_lib.lib().sap_plan_fwd_tiles(self._h))
+
+    def schedule(self, policy: int = 1):
+        """Compile Steps 2-3: (slots int32 [n_items, 2] = (rank, stage) per item, n_stages).  policy 0 = plain ring,
+        1 = balanced (SAP_SCHED_BALANCED)."""
+        slots = np.zeros((max(self.n_items, 1), 2), dtype=np.int32)
+        n_stages = ctypes.c_int32(0)
+        _check(_lib.lib().sap_plan_schedule(self._h, int(policy), slots.ctypes.data_as(ctypes.c_void_p),
+                                            ctypes.byref(n_stages)), "sap_plan_schedule")
+        return slots[:self.n_items], int(n_stages.value)
 
     def upload(self):
         _check(_lib.lib().sap_plan_upload(self._h), "sap_plan_upload")

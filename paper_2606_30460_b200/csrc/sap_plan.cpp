@@ -202,6 +202,74 @@ const uint8_t* sap_plan_kind_map(const sap_plan_t* p) { return p ? p->kind_map.d
 int64_t sap_plan_useful_pairs(const sap_plan_t* p) { return p ? p->useful_pairs : 0; }
 int64_t sap_plan_fwd_tiles(const sap_plan_t* p) { return p ? p->fwd.streamed_tiles : 0; }
 
+int sap_plan_schedule(const sap_plan_t* p, int32_t policy, sap_slot_t* slots, int32_t* n_stages) {
+  if (!p || !slots || !n_stages || (policy != SAP_SCHED_RING && policy != SAP_SCHED_BALANCED)) return SAP_ERR_INVALID_ARG;
+  const int32_t P = p->n_chunks, n_items = (int32_t)p->items.size();
+  const int64_t n = p->chunk_len;
+  int32_t last = 0;
+  if (policy == SAP_SCHED_RING) {
+    for (int32_t x = 0; x < n_items; ++x) {
+      slots[x].rank = p->items[x].q_chunk;
+      slots[x].stage = p->items[x].step;
+      last = std::max(last, slots[x].stage);
+    }
+    *n_stages = last + 1;
+    return SAP_OK;
+  }
+  // Step 2: regional strategy.  The region of a FULL item is its (single) document; it spans chunks a..b.
+  std::vector<int32_t> regional(n_items);
+  for (int32_t x = 0; x < n_items; ++x) {
+    const sap_item_t& im = p->items[x];
+    if (im.mask_kind == SAP_MASK_DIAG) { slots[x].rank = im.q_chunk; regional[x] = 0; continue; }
+    const int32_t e = im.doc_lo;
+    const int32_t a = (int32_t)(p->cu[e] / n), b = (int32_t)((p->cu[e + 1] - 1) / n), m = b - a + 1;
+    const int32_t t = im.q_chunk - im.kv_chunk;
+    if (t <= m / 2) { slots[x].rank = im.q_chunk; regional[x] = t; }
+    else            { slots[x].rank = im.kv_chunk; regional[x] = m - t; }
+  }
+  // Step 3a: global balance.  While the busiest rank (lowest index on ties) holds a FULL item whose other end is at
+  // least two items less loaded, hand over the one whose other end is least loaded (lowest item index on ties).
+  std::vector<int32_t> load(P, 0), dist_of(n_items, 0), span_of(n_items, 0);
+  for (int32_t x = 0; x < n_items; ++x) {
+    ++load[slots[x].rank];
+    const sap_item_t& im = p->items[x];
+    if (im.mask_kind == SAP_MASK_DIAG) continue;
+    const int32_t e = im.doc_lo;
+    span_of[x] = (int32_t)((p->cu[e + 1] - 1) / n) - (int32_t)(p->cu[e] / n) + 1;
+    dist_of[x] = im.q_chunk - im.kv_chunk;
+  }
+  for (;;) {
+    int32_t R = 0;
+    for (int32_t r = 1; r < P; ++r) if (load[r] > load[R]) R = r;
+    int32_t best = -1, best_other = -1;
+    for (int32_t x = 0; x < n_items; ++x) {
+      const sap_item_t& im = p->items[x];
+      if (slots[x].rank != R || im.mask_kind == SAP_MASK_DIAG) continue;
+      const int32_t other = (R == im.q_chunk) ? im.kv_chunk : im.q_chunk;
+      if (best < 0 || load[other] < load[best_other]) { best = x; best_other = other; }
+    }
+    if (best < 0 || load[best_other] + 1 >= load[R]) break;
+    --load[R]; ++load[best_other];
+    slots[best].rank = best_other;
+    regional[best] = (best_other == p->items[best].q_chunk) ? dist_of[best] : span_of[best] - dist_of[best];
+  }
+  // Step 3b: one item per rank per stage: every rank runs its items in order of (regional stage, q_chunk, kv_chunk)
+  std::vector<int32_t> order(n_items);
+  for (int32_t x = 0; x < n_items; ++x) order[x] = x;
+  std::stable_sort(order.begin(), order.end(), [&](int32_t x, int32_t y) {
+    if (regional[x] != regional[y]) return regional[x] < regional[y];
+    if (p->items[x].q_chunk != p->items[y].q_chunk) return p->items[x].q_chunk < p->items[y].q_chunk;
+    return p->items[x].kv_chunk < p->items[y].kv_chunk;
+  });
+  std::vector<int32_t> next_stage(P, 0);  // a rank runs its items back to back: stage = position in its sorted list
+  for (int32_t x : order) {
+    slots[x].stage = next_stage[slots[x].rank]++;
+    last = std::max(last, slots[x].stage);
+  }
+  *n_stages = last + 1;
+  return SAP_OK;
+}
+
 const char* sap_strerror(int status) {
   switch (status) {
     case SAP_OK: return "ok";
