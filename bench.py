@@ -240,16 +240,50 @@ def run_ours(args):
     r_out, r_lse = torch.empty_like(hq).pin_memory(), torch.empty((Hq, N), dtype=torch.float32).pin_memory()
     r_dq, r_dk, r_dv = torch.empty_like(hq).pin_memory(), torch.empty_like(hk).pin_memory(), torch.empty_like(hv).pin_memory()
 
-    def e2e_step():
-        q.copy_(hq, non_blocking=True); k.copy_(hk, non_blocking=True)
-        v.copy_(hv, non_blocking=True); do.copy_(hdo, non_blocking=True)
-        step()
-        r_out.copy_(out, non_blocking=True); r_lse.copy_(lse, non_blocking=True)
-        r_dq.copy_(dq, non_blocking=True); r_dk.copy_(dk, non_blocking=True); r_dv.copy_(dv, non_blocking=True)
+    # Double-buffered, three streams (a user's input pipeline): step i+1's inputs travel host -> device and step
+    # i-1's results device -> host while step i computes.  Every step still copies its own inputs from pinned host
+    # memory and reads its own results back; pipeline fill and drain are inside the timed region.
+    s_comp, s_h2d, s_d2h = torch.cuda.current_stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    d_in = [(q, k, v, do), tuple(torch.empty_like(x) for x in (q, k, v, do))]
+    d_out = [(out, lse, dq, dk, dv), tuple(torch.empty_like(x) for x in (out, lse, dq, dk, dv))]
+    h_in, h_out = (hq, hk, hv, hdo), (r_out, r_lse, r_dq, r_dk, r_dv)
 
-    e2e_step(); sync_all()
-    e_steps = max(2, min(args.steps, 5))
-    ms_e2e = timed(e2e_step, e_steps)
+    def e2e_run(n):
+        in_ready = [torch.cuda.Event() for _ in range(n)]
+        comp_done = [torch.cuda.Event() for _ in range(n)]
+        d2h_done = [torch.cuda.Event() for _ in range(n)]
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(s_h2d)
+        for i in range(n):
+            sl = i & 1
+            with torch.cuda.stream(s_h2d):
+                if i >= 2:
+                    s_h2d.wait_event(comp_done[i - 2])          # the slot's inputs have been consumed
+                for dst, src in zip(d_in[sl], h_in):
+                    dst.copy_(src, non_blocking=True)
+                in_ready[i].record(s_h2d)
+            s_comp.wait_event(in_ready[i])
+            if i >= 2:
+                s_comp.wait_event(d2h_done[i - 2])              # the slot's previous results have been read back
+            qi, ki, vi, doi = d_in[sl]
+            oi, li, dqi, dki, dvi = d_out[sl]
+            sap.sap_attn_fwd(qi, ki, vi, cu, plan, oi, li, softmax_scale=w.softmax_scale)
+            sap.sap_attn_bwd(doi, qi, ki, vi, oi, li, cu, plan, softmax_scale=w.softmax_scale, dq=dqi, dk=dki, dv=dvi,
+                             workspace=ws)
+            comp_done[i].record(s_comp)
+            with torch.cuda.stream(s_d2h):
+                s_d2h.wait_event(comp_done[i])
+                for dst, src in zip(h_out, d_out[sl]):
+                    dst.copy_(src, non_blocking=True)
+                d2h_done[i].record(s_d2h)
+        e1.record(s_d2h)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    e2e_run(2); sync_all()
+    e_steps = max(4, min(args.steps, 8))
+    ms_e2e = e2e_run(e_steps)
     sync_all()
     ms_e2e_max, _ = shard.aggregate(ms_e2e, 0.0, dev)
     e2e_value = flops_all / (ms_e2e_max * 1e-3) / 1e12
@@ -311,7 +345,8 @@ def run_ours(args):
             "bwd": {"ms": sum(per.values()), "tflops": w.flops_bwd / (sum(per.values()) * 1e-3) / 1e12},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "ms_per_step": ms_e2e_max},
+                    "ms_per_step": ms_e2e_max, "steps": e_steps,
+                    "pipeline": "double-buffered, 3 streams: H2D of step i+1 and D2H of step i-1 overlap step i"},
             "gpu_launches": int(launches),
             "roofline": roofline,
             "kernels": kernels,

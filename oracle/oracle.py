@@ -4,6 +4,10 @@ TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and
 bench.py's cpu_baseline / --impl reference leg may import this.  It imports nothing
 from paper_2606_30460_b200 (the CUDA path) and shares no code with it.
 
+Parity status: every float function and plan() are pinned (tests/test_oracle_*.py); schedule() (compile Steps 2-3)
+is PARTIALLY PINNED - validity, closed forms and bounds are pinned, the choice among valid schedules is a reading
+(R-5; the paper's Fig. 3 is missing).
+
 Arrays are numpy; Q/K/V/dO are float32 arrays holding bf16-exact values
 (`tensor.float().numpy()`); every result is float64.
 """
