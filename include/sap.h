@@ -103,6 +103,28 @@ enum { SAP_SCHED_RING = 0, SAP_SCHED_BALANCED = 1 };
 typedef struct { int32_t rank, stage; } sap_slot_t;
 int sap_plan_schedule(const sap_plan_t* plan, int32_t policy, sap_slot_t* slots, int32_t* n_stages);
 
+/* Jitted code generation (§3.2 :120-:124, instruction set of Table 1 :85-:98), forward pass: the
+ * instruction list of one rank for a schedule made by sap_plan_schedule.  One code = 5 x int32, memcmp-comparable:
+ *   stage   -1 (prologue) .. n_stages (epilogue); a rank walks its list in order, one stage after the other
+ *   opcode  SAP_OP_SEND / SAP_OP_RECV  create $send-op / $recv-op {tensor} %peer: all SEND/RECV codes of one stage form
+ *                                      ONE batched isend/irecv that is in flight while the stage's block is computed
+ *                                      (:122-:124); every SEND has its RECV at the same stage on the peer
+ *           SAP_OP_COMPUTING           partial attention of plan item `item` on the compute buffers (:102)
+ *           SAP_OP_COPY                after the stage's batch completed: received q / kv -> compute buffer; received
+ *                                      o -> merged into this rank's running (O, LSE) ("copy and rescale", :239)
+ *   tensor  SAP_T_Q / SAP_T_KV / SAP_T_O (o = a partial result: normalised output + LSE)
+ *   peer    the other rank (SEND: destination, RECV / COPY: source); -1 for COMPUTING
+ *   item    the plan item the data belongs to
+ * Rule: an item computed on the rank of its Q gets K/V_j sent j -> i one stage earlier; an item computed on the rank
+ * of its K/V (a helper, Step 2) gets Q_i sent i -> j one stage earlier and its partial result sent back j -> i one
+ * stage later.  Inside a stage: SEND / RECV codes ordered by (opcode, tensor, peer, item), then COMPUTING, then COPY
+ * codes ordered by (tensor, peer, item).
+ * codes: host, capacity `cap` codes; returns the number of codes of `rank` (call with cap = 0 to size), < 0 on error. */
+enum { SAP_OP_SEND = 0, SAP_OP_RECV = 1, SAP_OP_COMPUTING = 2, SAP_OP_COPY = 3 };
+enum { SAP_T_Q = 0, SAP_T_KV = 1, SAP_T_O = 2 };
+typedef struct { int32_t stage, opcode, tensor, peer, item; } sap_code_t;
+int32_t sap_plan_codegen(const sap_plan_t* plan, const sap_slot_t* slots, int32_t rank, sap_code_t* codes, int32_t cap);
+
 /* Copy the compiled work lists to the current CUDA device (cudaMalloc + synchronous cudaMemcpy).
  * Called implicitly by the first sap_attn_* call that uses the plan; call it yourself to keep that
  * cost out of a timed region.  Idempotent, thread-safe. */

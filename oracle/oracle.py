@@ -5,8 +5,9 @@ bench.py's cpu_baseline / --impl reference leg may import this.  It imports noth
 from paper_2606_30460_b200 (the CUDA path) and shares no code with it.
 
 Parity status: every float function and plan() are pinned (tests/test_oracle_*.py); schedule() (compile Steps 2-3)
-is PARTIALLY PINNED - validity, closed forms and bounds are pinned, the choice among valid schedules is a reading
-(R-5; the paper's Fig. 3 is missing).
+and codegen() (jitted code generation) are PARTIALLY PINNED - validity, closed forms, bounds, send/recv pairing and
+the replay test are pinned; the choice among valid schedules and the stage offsets are a reading (R-5; the
+paper's Fig. 3 is missing).
 
 Arrays are numpy; Q/K/V/dO are float32 arrays holding bf16-exact values
 (`tensor.float().numpy()`); every result is float64.
@@ -263,3 +264,42 @@ def schedule(cu_seqlens, n_chunks: int, policy: int = 1):
         slots[x, 1] = nxt[slots[x, 0]]          # a rank runs its items back to back in this order
         nxt[slots[x, 0]] += 1
     return slots, (int(slots[:, 1].max()) + 1 if len(items) else 0)
+
+
+OP_SEND, OP_RECV, OP_COMPUTING, OP_COPY = 0, 1, 2, 3
+T_Q, T_KV, T_O = 0, 1, 2
+
+
+def codegen(cu_seqlens, n_chunks: int, slots, rank: int):
+    """Jitted code generation for the forward pass (Table 1 :85-98), written out rule by rule.
+    Codes are (stage, opcode, tensor, peer, item).  For every plan item (i, j) with slot (R, st):
+      R runs `computing item` at stage st;
+      if i != j and R == i: kv travels j -> i at stage st-1 (send on j, recv + copy on i);
+      if i != j and R == j: q travels i -> j at stage st-1 (send on i, recv + copy on j) and the partial result o
+                            travels j -> i at stage st+1 (send on j, recv + copy-and-rescale on i).
+    Order inside a stage: SEND/RECV by (opcode, tensor, peer, item), then COMPUTING, then COPY by (tensor, peer, item).
+    PARITY: the transport rules above are the paper's (who needs which tensor follows from where the block runs);
+    the stage offsets (-1 / +1) and the order inside a stage are this build's reading - partially pinned: pinned by
+    the executor test (every rank's replay reproduces the unchunked attention) and by send/recv pairing."""
+    pl = plan(cu_seqlens, n_chunks)
+    out = []
+    for x, row in enumerate(pl.items):
+        i, j = int(row[0]), int(row[1])
+        R, st = int(slots[x][0]), int(slots[x][1])
+        if R == rank:
+            out.append((st, OP_COMPUTING, -1, -1, x))
+        if i == j:
+            continue
+        if R == i:
+            if rank == j:
+                out.append((st - 1, OP_SEND, T_KV, i, x))
+            if rank == i:
+                out += [(st - 1, OP_RECV, T_KV, j, x), (st - 1, OP_COPY, T_KV, j, x)]
+        else:
+            if rank == i:
+                out += [(st - 1, OP_SEND, T_Q, j, x), (st + 1, OP_RECV, T_O, j, x), (st + 1, OP_COPY, T_O, j, x)]
+            if rank == j:
+                out += [(st - 1, OP_RECV, T_Q, i, x), (st - 1, OP_COPY, T_Q, i, x), (st + 1, OP_SEND, T_O, i, x)]
+    phase = {OP_SEND: 0, OP_RECV: 0, OP_COMPUTING: 1, OP_COPY: 2}
+    out.sort(key=lambda c: (c[0], phase[c[1]], c[1] if phase[c[1]] == 0 else 0, c[2], c[3], c[4]))
+    return np.array(out, dtype=np.int32).reshape(-1, 5)

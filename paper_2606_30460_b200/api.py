@@ -12,6 +12,8 @@ from . import _lib
 SAP_MASK_SKIP, SAP_MASK_FULL, SAP_MASK_DIAG = 0, 1, 2
 SAP_PASS_FWD, SAP_PASS_BWD = 0, 1
 SAP_SCHED_RING, SAP_SCHED_BALANCED = 0, 1
+SAP_OP_SEND, SAP_OP_RECV, SAP_OP_COMPUTING, SAP_OP_COPY = 0, 1, 2, 3
+SAP_T_Q, SAP_T_KV, SAP_T_O = 0, 1, 2
 
 
 class SapError(RuntimeError):
@@ -111,6 +113,17 @@ class Plan:
         _check(_lib.lib().sap_plan_schedule(self._h, int(policy), slots.ctypes.data_as(ctypes.c_void_p),
                                             ctypes.byref(n_stages)), "sap_plan_schedule")
         return slots[:self.n_items], int(n_stages.value)
+
+    def codegen(self, slots: np.ndarray, rank: int) -> np.ndarray:
+        """Jitted code generation: int32 [n_codes, 5] = (stage, opcode, tensor, peer, item) of `rank` (sap_code_t)."""
+        L = _lib.lib()
+        sl = np.ascontiguousarray(slots, dtype=np.int32)
+        n = int(L.sap_plan_codegen(self._h, sl.ctypes.data_as(ctypes.c_void_p), int(rank), None, 0))
+        if n < 0:
+            raise SapError(-n, "sap_plan_codegen")
+        codes = np.zeros((max(n, 1), 5), dtype=np.int32)
+        L.sap_plan_codegen(self._h, sl.ctypes.data_as(ctypes.c_void_p), int(rank), codes.ctypes.data_as(ctypes.c_void_p), n)
+        return codes[:n]
 
     def upload(self):
         _check(_lib.lib().sap_plan_upload(self._h), "sap_plan_upload")

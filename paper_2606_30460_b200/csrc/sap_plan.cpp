@@ -270,6 +270,40 @@ int sap_plan_schedule(const sap_plan_t* p, int32_t policy, sap_slot_t* slots, in
   return SAP_OK;
 }
 
+int32_t sap_plan_codegen(const sap_plan_t* p, const sap_slot_t* slots, int32_t rank, sap_code_t* codes, int32_t cap) {
+  if (!p || !slots || rank < 0 || rank >= p->n_chunks || cap < 0 || (cap > 0 && !codes)) return -SAP_ERR_INVALID_ARG;
+  const int32_t n_items = (int32_t)p->items.size();
+  std::vector<sap_code_t> out;
+  for (int32_t x = 0; x < n_items; ++x) {
+    const sap_item_t& im = p->items[x];
+    const int32_t i = im.q_chunk, j = im.kv_chunk, R = slots[x].rank, st = slots[x].stage;
+    if (R != i && R != j) return -SAP_ERR_INVALID_ARG;
+    if (R == rank) out.push_back({st, SAP_OP_COMPUTING, -1, -1, x});
+    if (i == j) continue;
+    if (R == i) {  // K/V_j travels j -> i one stage earlier
+      if (rank == j) out.push_back({st - 1, SAP_OP_SEND, SAP_T_KV, i, x});
+      if (rank == i) { out.push_back({st - 1, SAP_OP_RECV, SAP_T_KV, j, x}); out.push_back({st - 1, SAP_OP_COPY, SAP_T_KV, j, x}); }
+    } else {       // helper: Q_i travels i -> j one stage earlier, the partial result j -> i one stage later
+      if (rank == i) out.push_back({st - 1, SAP_OP_SEND, SAP_T_Q, j, x});
+      if (rank == j) { out.push_back({st - 1, SAP_OP_RECV, SAP_T_Q, i, x}); out.push_back({st - 1, SAP_OP_COPY, SAP_T_Q, i, x}); }
+      if (rank == j) out.push_back({st + 1, SAP_OP_SEND, SAP_T_O, i, x});
+      if (rank == i) { out.push_back({st + 1, SAP_OP_RECV, SAP_T_O, j, x}); out.push_back({st + 1, SAP_OP_COPY, SAP_T_O, j, x}); }
+    }
+  }
+  auto phase = [](const sap_code_t& c) { return c.opcode <= SAP_OP_RECV ? 0 : (c.opcode == SAP_OP_COMPUTING ? 1 : 2); };
+  std::stable_sort(out.begin(), out.end(), [&](const sap_code_t& a, const sap_code_t& b) {
+    if (a.stage != b.stage) return a.stage < b.stage;
+    if (phase(a) != phase(b)) return phase(a) < phase(b);
+    if (phase(a) == 0 && a.opcode != b.opcode) return a.opcode < b.opcode;
+    if (a.tensor != b.tensor) return a.tensor < b.tensor;
+    if (a.peer != b.peer) return a.peer < b.peer;
+    return a.item < b.item;
+  });
+  const int32_t n = (int32_t)out.size();
+  for (int32_t c = 0; c < n && c < cap; ++c) codes[c] = out[c];
+  return n;
+}
+
 const char* sap_strerror(int status) {
   switch (status) {
     case SAP_OK: return "ok";
