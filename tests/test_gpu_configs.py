@@ -27,7 +27,7 @@ from parity import check_close, check_lse, to_np
 pytestmark = pytest.mark.gpu
 
 # cfg -> (kv-heads the oracle checks, random rows, live rows of the sparse-dO pass)
-PLAN = {2: ((0, 3, 7), 256, 256), 3: ((1, 6), 160, 192), 4: ((5,), 96, 128), 5: ((2,), 128, 160)}
+PLAN = {2: ((0, 3, 7), 512, 512), 3: ((1, 6), 384, 384), 4: ((5,), 256, 256), 5: ((2,), 256, 320)}
 
 
 def sample_rows(w, n_random, rng):
@@ -50,8 +50,8 @@ def sample_cols(w, rng):
     docs = sorted(range(len(w.doc_lens)), key=lambda e: -w.doc_lens[e])
     cols = set()
     for e in docs[:4]:                       # tail window of the longest documents
-        cols.update(range(max(cu[e], cu[e + 1] - 40), cu[e + 1]))
-    short = [e for e in docs if 0 < w.doc_lens[e] <= 768][:4]
+        cols.update(range(max(cu[e], cu[e + 1] - 96), cu[e + 1]))
+    short = [e for e in docs if 0 < w.doc_lens[e] <= 768][:6]
     for e in short:                          # whole short documents
         cols.update(range(cu[e], cu[e + 1]))
     return np.array(sorted(cols), dtype=np.int64)
