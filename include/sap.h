@@ -179,6 +179,37 @@ int sap_attn_bwd(const void* dout, const void* q, const void* k, const void* v, 
                  int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
                  void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* ---- per-rank launches ------------------------------------------------------------------
+ * The same kernels restricted to the chunks one rank owns (rank i holds Q_i, K_i, V_i).  Token indices
+ * stay global: every pointer is the base of the WHOLE [N, H, d] tensor, of which a launch reads the rows the plan
+ * names and writes only the rows of its own chunks.  With the tensors laid out across GPUs (peer-mapped virtual
+ * memory), a rank's forward streams the K/V tiles of other ranks through TMA while it computes, and a rank's
+ * backward adds its dQ contributions into the owner's accumulator with red.global - the transfer is inside the
+ * kernel, tile by tile.  On one GPU the chunk ranges simply partition one launch into P launches.
+ *
+ * sap_attn_fwd_chunks : forward of q-chunks [q_chunk_begin, q_chunk_end): writes out / lse rows of those chunks only.
+ * Backward in three phases that ranks run with a barrier in between (workspace as for sap_attn_bwd; all three take
+ * the base of the whole workspace):
+ *   sap_attn_bwd_begin  : D = rowsum(dO * O) for the rows of q-chunks [begin, end) and zeroes their dQ accumulator rows
+ *   sap_attn_bwd_chunks : fused kernel for the K/V tiles of kv-chunks [begin, end): writes dk / dv rows of those
+ *                         chunks, adds dQ contributions into the accumulator rows of every q-chunk that attends them;
+ *                         needs chunk_len % 128 == 0 (SAP_ERR_UNSUPPORTED otherwise)
+ *   sap_attn_bwd_end    : dq rows of q-chunks [begin, end) = bf16(scale * accumulator)
+ * All asynchronous on cuda_stream; device pointers as in sap_attn_fwd / sap_attn_bwd. */
+int sap_attn_fwd_chunks(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev, sap_plan_t* plan,
+                        int32_t q_chunk_begin, int32_t q_chunk_end, void* out, float* lse,
+                        int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale, void* cuda_stream);
+int sap_attn_bwd_begin(const void* dout, const void* out, sap_plan_t* plan, int32_t q_chunk_begin, int32_t q_chunk_end,
+                       int n_q_heads, int n_kv_heads, int head_dim, void* workspace, size_t workspace_bytes,
+                       void* cuda_stream);
+int sap_attn_bwd_chunks(const void* dout, const void* q, const void* k, const void* v, const float* lse,
+                        const int32_t* cu_seqlens_dev, sap_plan_t* plan, int32_t kv_chunk_begin, int32_t kv_chunk_end,
+                        void* dk, void* dv, int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
+                        void* workspace, size_t workspace_bytes, void* cuda_stream);
+int sap_attn_bwd_end(sap_plan_t* plan, int32_t q_chunk_begin, int32_t q_chunk_end, void* dq,
+                     int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* ---- diagnostics ---------------------------------------------------------------------------- */
 const char* sap_strerror(int status);
 int sap_last_cuda_error(void);      /* the cudaError_t / CUresult of the last SAP_ERR_CUDA on this thread */

@@ -233,3 +233,43 @@ def sap_debug_set_bwd_stages(mask: int) -> int:
 def sap_debug_set_fwd_form(form: int) -> int:
     """Diagnostic: 0 = pair forward kernel when Hq/Hkv is even (default), 1 = always the one-head kernel."""
     return int(_lib.lib().sap_debug_set_fwd_form(int(form)))
+
+
+# ---- per-rank launches (SURVEY 8(f) NEXT-1): the same kernels restricted to the chunks one rank owns ----------------
+def sap_attn_fwd_chunks(q, k, v, cu_seqlens_dev, plan: Plan, q_chunk_begin: int, q_chunk_end: int, out, lse,
+                        softmax_scale: Optional[float] = None, stream=None):
+    """Forward of q-chunks [q_chunk_begin, q_chunk_end): writes only those rows of out [N,Hq,d] / lse [Hq,N]."""
+    _require_cuda_bf16(q, k, v, out)
+    N, Hq, Hkv, d = _dims(q, k)
+    scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
+    _check(_lib.lib().sap_attn_fwd_chunks(_ptr(q), _ptr(k), _ptr(v), _ptr(cu_seqlens_dev), plan.handle,
+                                          int(q_chunk_begin), int(q_chunk_end), _ptr(out), _ptr(lse), Hq, Hkv, d, scale,
+                                          _stream(stream)), "sap_attn_fwd_chunks")
+    return out, lse
+
+
+def sap_attn_bwd_begin(dout, out, plan: Plan, q_chunk_begin: int, q_chunk_end: int, n_kv_heads: int, workspace, stream=None):
+    N, Hq, d = dout.shape
+    _check(_lib.lib().sap_attn_bwd_begin(_ptr(dout), _ptr(out), plan.handle, int(q_chunk_begin), int(q_chunk_end),
+                                         int(Hq), int(n_kv_heads), int(d), _ptr(workspace), workspace.numel(),
+                                         _stream(stream)), "sap_attn_bwd_begin")
+
+
+def sap_attn_bwd_chunks(dout, q, k, v, lse, cu_seqlens_dev, plan: Plan, kv_chunk_begin: int, kv_chunk_end: int, dk, dv,
+                        workspace, softmax_scale: Optional[float] = None, stream=None):
+    _require_cuda_bf16(dout, q, k, v, dk, dv)
+    N, Hq, Hkv, d = _dims(q, k)
+    scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
+    _check(_lib.lib().sap_attn_bwd_chunks(_ptr(dout), _ptr(q), _ptr(k), _ptr(v), _ptr(lse), _ptr(cu_seqlens_dev),
+                                          plan.handle, int(kv_chunk_begin), int(kv_chunk_end), _ptr(dk), _ptr(dv), Hq, Hkv,
+                                          d, scale, _ptr(workspace), workspace.numel(), _stream(stream)),
+           "sap_attn_bwd_chunks")
+
+
+def sap_attn_bwd_end(plan: Plan, q_chunk_begin: int, q_chunk_end: int, dq, n_kv_heads: int, workspace,
+                     softmax_scale: Optional[float] = None, stream=None):
+    N, Hq, d = dq.shape
+    scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
+    _check(_lib.lib().sap_attn_bwd_end(plan.handle, int(q_chunk_begin), int(q_chunk_end), _ptr(dq), int(Hq),
+                                       int(n_kv_heads), int(d), scale, _ptr(workspace), workspace.numel(),
+                                       _stream(stream)), "sap_attn_bwd_end")

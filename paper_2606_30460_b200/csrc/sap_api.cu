@@ -135,7 +135,7 @@ static int launch_bwd(const PlanDevice* pd, const void* dout, const void* q, con
     const int64_t want = (rows * (D / 8) + kPreThreads - 1) / kPreThreads;
     const unsigned grid = static_cast<unsigned>(want < 148 * 16 ? want : 148 * 16);
     sap_bwd_pre_kernel<D><<<grid, kPreThreads, 0, stream>>>(static_cast<const __nv_bfloat16*>(dout),
-                                                            static_cast<const __nv_bfloat16*>(out), dsum, N, Hq);
+                                                            static_cast<const __nv_bfloat16*>(out), dsum, N, Hq, 0, N);
     g_launch_count.fetch_add(1);
     SAP_CUDA_CHECK(cudaGetLastError());
   }
@@ -191,6 +191,81 @@ static int launch_bwd(const PlanDevice* pd, const void* dout, const void* q, con
   return SAP_OK;
 }
 
+// ---- pieces of the backward for chunk-restricted launches (sap_attn_bwd_begin / _chunks / _end) ----------------
+template <int D>
+static int launch_bwd_begin(const void* dout, const void* out, int64_t N, int Hq, int64_t t0, int64_t nt, float* dsum,
+                            float* dq_acc, cudaStream_t stream) {
+  const int64_t want = (nt * Hq * (D / 8) + kPreThreads - 1) / kPreThreads;
+  const unsigned grid = static_cast<unsigned>(want < 148 * 16 ? want : 148 * 16);
+  sap_bwd_pre_kernel<D><<<grid, kPreThreads, 0, stream>>>(static_cast<const __nv_bfloat16*>(dout),
+                                                          static_cast<const __nv_bfloat16*>(out), dsum, N, Hq, t0, nt);
+  g_launch_count.fetch_add(1);
+  SAP_CUDA_CHECK(cudaGetLastError());
+  SAP_CUDA_CHECK(cudaMemsetAsync(dq_acc + t0 * Hq * D, 0, static_cast<size_t>(nt) * Hq * D * sizeof(float), stream));
+  return SAP_OK;
+}
+
+template <int D>
+static int launch_bwd_fused_program(const DevProgram& prog, const void* dout, const void* q, const void* k, const void* v,
+                                    const float* lse, const int32_t* cu, const sap_plan_t* plan, void* dk, void* dv, int Hq,
+                                    int Hkv, float scale, const float* dsum, float* dq_acc, cudaStream_t stream) {
+  const int64_t N = plan->n_tokens;
+  CUtensorMap mq64, mdo64, mk128, mv128;
+  int rc;
+  if ((rc = make_tile_map(&mq64, q, N, (int64_t)Hq * D, kBwdN)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mdo64, dout, N, (int64_t)Hq * D, kBwdN)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mk128, k, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mv128, v, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
+  static bool attr_set = false;
+  if (!attr_set) {
+    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_fused_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FusedSmem<D>::kTotal));
+    attr_set = true;
+  }
+  if (prog.n_tiles == 0) return SAP_OK;
+  sap_bwd_fused_kernel<D><<<static_cast<unsigned>(prog.n_tiles) * Hkv, kFusedThreads, FusedSmem<D>::kTotal, stream>>>(
+      mq64, mdo64, mk128, mv128, prog.tiles, prog.segs, cu, plan->n_docs, lse, dsum, dq_acc,
+      static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
+  g_launch_count.fetch_add(1);
+  SAP_CUDA_CHECK(cudaGetLastError());
+  return SAP_OK;
+}
+
+static int launch_bwd_end(const float* dq_acc, void* dq, int Hq, int d, int64_t t0, int64_t nt, float scale, cudaStream_t stream) {
+  const int64_t n8 = nt * Hq * d / 8;
+  if (n8 == 0) return SAP_OK;
+  const int64_t want = (n8 + kPostThreads - 1) / kPostThreads;
+  const unsigned grid = static_cast<unsigned>(want < 148 * 16 ? want : 148 * 16);
+  sap_bwd_post_kernel<<<grid, kPostThreads, 0, stream>>>(dq_acc + t0 * Hq * d,
+                                                         static_cast<__nv_bfloat16*>(dq) + t0 * Hq * d, n8, scale);
+  g_launch_count.fetch_add(1);
+  SAP_CUDA_CHECK(cudaGetLastError());
+  return SAP_OK;
+}
+
+// item-range (forward) or kv-chunk-range (backward) restricted programs, built once per range and kept with the plan
+static int get_chunk_program(sap_plan_t* plan, bool kv, int32_t c_begin, int32_t c_end, DevProgram* out) {
+  PlanDevice* pd = static_cast<PlanDevice*>(plan->dev_state);
+  std::lock_guard<std::mutex> lock(plan->mu);
+  auto& cache = kv ? pd->kv_chunks : pd->q_chunks;
+  auto key = std::make_pair(c_begin, c_end);
+  auto itp = cache.find(key);
+  if (itp == cache.end()) {
+    TileProgram host;
+    if (kv) build_kv_program(*plan, host, c_begin, c_end);
+    else build_q_program(*plan, plan->chunk_offsets[c_begin], plan->chunk_offsets[c_end], host, /*drop_empty=*/true);
+    DevProgram dp;
+    int rc = upload_program(host, dp);
+    if (rc != SAP_OK) return rc;
+    itp = cache.emplace(key, dp).first;
+  }
+  *out = itp->second;
+  return SAP_OK;
+}
+
+static inline bool chunk_range_ok(const sap_plan_t* plan, int32_t a, int32_t b) {
+  return a >= 0 && b >= a && b <= plan->n_chunks;
+}
+
 }  // namespace sap
 
 using namespace sap;
@@ -229,6 +304,8 @@ void sap_plan_destroy(sap_plan_t* plan) {
     free_program(pd->fwd);
     free_program(pd->kv);
     for (auto& kv : pd->partial) free_program(kv.second);
+    for (auto& kv : pd->q_chunks) free_program(kv.second);
+    for (auto& kv : pd->kv_chunks) free_program(kv.second);
     delete pd;
   }
   delete plan;
@@ -336,6 +413,87 @@ int sap_attn_bwd(const void* dout, const void* q, const void* k, const void* v, 
                            softmax_scale, dsum, dq_acc, st);
   return launch_bwd<64>(pd, dout, q, k, v, out, lse, cu_seqlens_dev, plan, dq, dk, dv, n_q_heads, n_kv_heads,
                         softmax_scale, dsum, dq_acc, st);
+}
+
+int sap_attn_fwd_chunks(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev, sap_plan_t* plan,
+                        int32_t q_chunk_begin, int32_t q_chunk_end, void* out, float* lse, int n_q_heads, int n_kv_heads,
+                        int head_dim, float softmax_scale, void* cuda_stream) {
+  if (!q || !k || !v || !cu_seqlens_dev || !out || !lse) return SAP_ERR_INVALID_ARG;
+  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  if (rc != SAP_OK) return rc;
+  if (!chunk_range_ok(plan, q_chunk_begin, q_chunk_end)) return SAP_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out)) return SAP_ERR_UNSUPPORTED;
+  if ((rc = sap_plan_upload(plan)) != SAP_OK) return rc;
+  if (q_chunk_begin == q_chunk_end) return SAP_OK;
+  DevProgram prog;
+  if ((rc = get_chunk_program(plan, false, q_chunk_begin, q_chunk_end, &prog)) != SAP_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (head_dim == 128)
+    return launch_fwd<128, false>(prog, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st);
+  return launch_fwd<64, false>(prog, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st);
+}
+
+static int bwd_ws(const sap_plan_t* plan, int Hq, int Hkv, int d, void* workspace, size_t bytes, float** dsum, float** dq_acc) {
+  if (!aligned16(workspace)) return SAP_ERR_UNSUPPORTED;
+  if (!workspace || bytes < sap_workspace_bytes(plan, Hq, Hkv, d, SAP_PASS_BWD)) return SAP_ERR_WORKSPACE_TOO_SMALL;
+  *dsum = static_cast<float*>(workspace);
+  *dq_acc = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + align256(static_cast<size_t>(plan->n_tokens) * Hq * sizeof(float)));
+  return SAP_OK;
+}
+
+int sap_attn_bwd_begin(const void* dout, const void* out, sap_plan_t* plan, int32_t q_chunk_begin, int32_t q_chunk_end,
+                       int n_q_heads, int n_kv_heads, int head_dim, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!dout || !out) return SAP_ERR_INVALID_ARG;
+  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, 1.f);
+  if (rc != SAP_OK) return rc;
+  if (!chunk_range_ok(plan, q_chunk_begin, q_chunk_end)) return SAP_ERR_INVALID_ARG;
+  if (!aligned16(dout) || !aligned16(out)) return SAP_ERR_UNSUPPORTED;
+  float *dsum, *dq_acc;
+  if ((rc = bwd_ws(plan, n_q_heads, n_kv_heads, head_dim, workspace, workspace_bytes, &dsum, &dq_acc)) != SAP_OK) return rc;
+  if ((rc = check_device_is_sm100()) != SAP_OK) return rc;
+  const int64_t t0 = (int64_t)q_chunk_begin * plan->chunk_len, nt = (int64_t)(q_chunk_end - q_chunk_begin) * plan->chunk_len;
+  if (nt == 0) return SAP_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (head_dim == 128) return launch_bwd_begin<128>(dout, out, plan->n_tokens, n_q_heads, t0, nt, dsum, dq_acc, st);
+  return launch_bwd_begin<64>(dout, out, plan->n_tokens, n_q_heads, t0, nt, dsum, dq_acc, st);
+}
+
+int sap_attn_bwd_chunks(const void* dout, const void* q, const void* k, const void* v, const float* lse,
+                        const int32_t* cu_seqlens_dev, sap_plan_t* plan, int32_t kv_chunk_begin, int32_t kv_chunk_end,
+                        void* dk, void* dv, int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
+                        void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!dout || !q || !k || !v || !lse || !cu_seqlens_dev || !dk || !dv) return SAP_ERR_INVALID_ARG;
+  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  if (rc != SAP_OK) return rc;
+  if (!chunk_range_ok(plan, kv_chunk_begin, kv_chunk_end)) return SAP_ERR_INVALID_ARG;
+  if (plan->chunk_len % kTile != 0) return SAP_ERR_UNSUPPORTED;  // K/V tiles must not straddle two ranks' chunks
+  if (!aligned16(dout) || !aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(dk) || !aligned16(dv)) return SAP_ERR_UNSUPPORTED;
+  float *dsum, *dq_acc;
+  if ((rc = bwd_ws(plan, n_q_heads, n_kv_heads, head_dim, workspace, workspace_bytes, &dsum, &dq_acc)) != SAP_OK) return rc;
+  if ((rc = sap_plan_upload(plan)) != SAP_OK) return rc;
+  if (kv_chunk_begin == kv_chunk_end) return SAP_OK;
+  DevProgram prog;
+  if ((rc = get_chunk_program(plan, true, kv_chunk_begin, kv_chunk_end, &prog)) != SAP_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (head_dim == 128)
+    return launch_bwd_fused_program<128>(prog, dout, q, k, v, lse, cu_seqlens_dev, plan, dk, dv, n_q_heads, n_kv_heads,
+                                         softmax_scale, dsum, dq_acc, st);
+  return launch_bwd_fused_program<64>(prog, dout, q, k, v, lse, cu_seqlens_dev, plan, dk, dv, n_q_heads, n_kv_heads,
+                                      softmax_scale, dsum, dq_acc, st);
+}
+
+int sap_attn_bwd_end(sap_plan_t* plan, int32_t q_chunk_begin, int32_t q_chunk_end, void* dq, int n_q_heads, int n_kv_heads,
+                     int head_dim, float softmax_scale, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!dq) return SAP_ERR_INVALID_ARG;
+  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  if (rc != SAP_OK) return rc;
+  if (!chunk_range_ok(plan, q_chunk_begin, q_chunk_end)) return SAP_ERR_INVALID_ARG;
+  if (!aligned16(dq)) return SAP_ERR_UNSUPPORTED;
+  float *dsum, *dq_acc;
+  if ((rc = bwd_ws(plan, n_q_heads, n_kv_heads, head_dim, workspace, workspace_bytes, &dsum, &dq_acc)) != SAP_OK) return rc;
+  if ((rc = check_device_is_sm100()) != SAP_OK) return rc;
+  const int64_t t0 = (int64_t)q_chunk_begin * plan->chunk_len, nt = (int64_t)(q_chunk_end - q_chunk_begin) * plan->chunk_len;
+  return launch_bwd_end(dq_acc, dq, n_q_heads, head_dim, t0, nt, softmax_scale, static_cast<cudaStream_t>(cuda_stream));
 }
 
 }  // extern "C"

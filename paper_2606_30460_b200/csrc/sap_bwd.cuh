@@ -25,9 +25,11 @@ constexpr int kPreThreads = 256;
 template <int D>
 __global__ void __launch_bounds__(kPreThreads)
 sap_bwd_pre_kernel(const __nv_bfloat16* __restrict__ dout, const __nv_bfloat16* __restrict__ out,
-                   float* __restrict__ dsum, int64_t n_tokens, int n_q_heads) {
+                   float* __restrict__ dsum, int64_t n_tokens, int n_q_heads, int64_t token_begin, int64_t token_count) {
   constexpr int G = D / 8;  // lanes per row, 8 bf16 each
-  const int64_t n_rows = n_tokens * n_q_heads;
+  dout += token_begin * n_q_heads * D;   // tokens [token_begin, token_begin + token_count) only
+  out += token_begin * n_q_heads * D;
+  const int64_t n_rows = token_count * n_q_heads;
   const int64_t gthread = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x;
   const int64_t groups_total = static_cast<int64_t>(gridDim.x) * blockDim.x / G;
   const int gl = static_cast<int>(gthread % G);
@@ -47,7 +49,7 @@ sap_bwd_pre_kernel(const __nv_bfloat16* __restrict__ dout, const __nv_bfloat16* 
 #pragma unroll
     for (int o = G / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
     if (row < n_rows && gl == 0) {
-      const int64_t t = row / n_q_heads;
+      const int64_t t = token_begin + row / n_q_heads;
       const int h = static_cast<int>(row % n_q_heads);
       dsum[h * n_tokens + t] = acc;
     }

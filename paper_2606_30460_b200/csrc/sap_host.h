@@ -34,6 +34,7 @@ struct PlanDevice {
   int device = -1;
   DevProgram fwd, kv;
   std::map<std::pair<int32_t, int32_t>, DevProgram> partial;  // item-range-restricted Q programs
+  std::map<std::pair<int32_t, int32_t>, DevProgram> q_chunks, kv_chunks;  // chunk-range-restricted programs (per-rank launches)
 };
 
 int check_device_is_sm100();

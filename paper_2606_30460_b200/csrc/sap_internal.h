@@ -51,6 +51,8 @@ struct sap_plan {
 
 namespace sap {
 // Build a Q-stationary tile program restricted to items [item_begin, item_end).
-void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, TileProgram& out);
-void build_kv_program(const sap_plan& p, TileProgram& out);
+// `drop_empty`: leave out tiles that have no work among those items (a rank's launch touches only its own rows).
+void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, TileProgram& out, bool drop_empty = false);
+// K/V tiles of kv-chunks [chunk_begin, chunk_end) only (the whole sequence by default).
+void build_kv_program(const sap_plan& p, TileProgram& out, int32_t chunk_begin = 0, int32_t chunk_end = -1);
 }  // namespace sap

@@ -26,7 +26,7 @@ static inline int32_t doc_of(const std::vector<int32_t>& cu, int64_t t) {
 
 static inline int32_t floor_tile(int64_t x) { return (int32_t)(x / kTile * kTile); }
 
-void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, TileProgram& out) {
+void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, TileProgram& out, bool drop_empty) {
   out.tiles.clear();
   out.segs.clear();
   out.streamed_tiles = 0;
@@ -60,6 +60,7 @@ void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, Ti
         w += (hi - sd.t_begin + kTile - 1) / kTile;
       }
       td.seg_end = (int32_t)out.segs.size();
+      if (drop_empty && td.seg_end == td.seg_begin) continue;
       out.tiles.push_back(td);
       work.push_back(w);
       out.streamed_tiles += w;
@@ -74,7 +75,7 @@ void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, Ti
   out.tiles.swap(sorted);
 }
 
-void build_kv_program(const sap_plan& p, TileProgram& out) {
+void build_kv_program(const sap_plan& p, TileProgram& out, int32_t chunk_begin, int32_t chunk_end) {
   out.tiles.clear();
   out.segs.clear();
   out.streamed_tiles = 0;
@@ -82,8 +83,9 @@ void build_kv_program(const sap_plan& p, TileProgram& out) {
   std::vector<int64_t> work;
   // K/V tiles are globally 128-aligned (they must match the key tiles the forward kernel streams only in
   // coverage, not in alignment); a tile that straddles two kv-chunks gets segments from both.
-  for (int64_t c0 = 0; c0 < N; c0 += kTile) {
-    const int64_t c1 = std::min<int64_t>(c0 + kTile, N);
+  const int64_t k_begin = (int64_t)chunk_begin * n, k_end = chunk_end < 0 ? N : (int64_t)chunk_end * n;  // 128-aligned when restricted
+  for (int64_t c0 = k_begin; c0 < k_end; c0 += kTile) {
+    const int64_t c1 = std::min<int64_t>(c0 + kTile, k_end);
     TileDesc td;
     td.row0 = (int32_t)c0;
     td.rows = (int32_t)(c1 - c0);
