@@ -34,6 +34,8 @@ CASES = {
     "chunk_not_tile_multiple": ([300, 33, 167], 5, 4, 2, 64),
     "gqa_4_several_tiles": ([700, 1100, 248 + 512], 5, 8, 2, 128),
     "doc_starts_at_chunk_boundary": ([512, 512, 1024], 4, 2, 2, 64),
+    "gqa_3_odd_group": ([300, 500, 96], 2, 6, 2, 128),
+    "gqa_6_three_pairs": ([640, 384], 4, 6, 1, 64),
 }
 
 
