@@ -125,6 +125,15 @@ enum { SAP_T_Q = 0, SAP_T_KV = 1, SAP_T_O = 2 };
 typedef struct { int32_t stage, opcode, tensor, peer, item; } sap_code_t;
 int32_t sap_plan_codegen(const sap_plan_t* plan, const sap_slot_t* slots, int32_t rank, sap_code_t* codes, int32_t cap);
 
+/* The same for the backward pass (tensors do / dq / dkv of Table 1).  An item computed on the rank of
+ * its Q (which also holds dO, LSE and D of those rows) gets K/V_j sent j -> i one stage earlier and sends its dK/dV
+ * contribution (`dkv`) back j <- i one stage later; an item computed on the rank of its K/V gets Q_i and dO_i (`do`
+ * carries LSE and D along) one stage earlier and sends its dQ contribution (`dq`) back to i one stage later.  COPY of
+ * a received dq / dkv adds it into the owner's gradient.  Same code format, order and return value as
+ * sap_plan_codegen; tensors SAP_T_Q, SAP_T_KV, SAP_T_DO, SAP_T_DQ, SAP_T_DKV. */
+enum { SAP_T_DO = 3, SAP_T_DQ = 4, SAP_T_DKV = 5 };
+int32_t sap_plan_codegen_bwd(const sap_plan_t* plan, const sap_slot_t* slots, int32_t rank, sap_code_t* codes, int32_t cap);
+
 /* Copy the compiled work lists to the current CUDA device (cudaMalloc + synchronous cudaMemcpy).
  * Called implicitly by the first sap_attn_* call that uses the plan; call it yourself to keep that
  * cost out of a timed region.  Idempotent, thread-safe. */

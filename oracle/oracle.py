@@ -303,3 +303,70 @@ def codegen(cu_seqlens, n_chunks: int, slots, rank: int):
     phase = {OP_SEND: 0, OP_RECV: 0, OP_COMPUTING: 1, OP_COPY: 2}
     out.sort(key=lambda c: (c[0], phase[c[1]], c[1] if phase[c[1]] == 0 else 0, c[2], c[3], c[4]))
     return np.array(out, dtype=np.int32).reshape(-1, 5)
+
+
+T_DO, T_DQ, T_DKV = 3, 4, 5
+
+
+def codegen_bwd(cu_seqlens, n_chunks: int, slots, rank: int):
+    """Backward instruction list of `rank` (tensors do / dq / dkv of Table 1), rule by rule:
+      R == i: kv travels j -> i at stage st-1, the dK/dV contribution (dkv) travels i -> j at stage st+1;
+      R == j: q and do (with LSE, D) travel i -> j at stage st-1, the dQ contribution (dq) travels j -> i at st+1.
+    Same format and order as codegen().  Partially pinned, as codegen()."""
+    pl = plan(cu_seqlens, n_chunks)
+    out = []
+
+    def transfer(stage, tensor, src, dst, x):
+        if rank == src:
+            out.append((stage, OP_SEND, tensor, dst, x))
+        if rank == dst:
+            out.extend([(stage, OP_RECV, tensor, src, x), (stage, OP_COPY, tensor, src, x)])
+
+    for x, row in enumerate(pl.items):
+        i, j = int(row[0]), int(row[1])
+        R, st = int(slots[x][0]), int(slots[x][1])
+        if R == rank:
+            out.append((st, OP_COMPUTING, -1, -1, x))
+        if i == j:
+            continue
+        if R == i:
+            transfer(st - 1, T_KV, j, i, x)
+            transfer(st + 1, T_DKV, i, j, x)
+        else:
+            transfer(st - 1, T_Q, i, j, x)
+            transfer(st - 1, T_DO, i, j, x)
+            transfer(st + 1, T_DQ, j, i, x)
+    phase = {OP_SEND: 0, OP_RECV: 0, OP_COMPUTING: 1, OP_COPY: 2}
+    out.sort(key=lambda c: (c[0], phase[c[1]], c[1] if phase[c[1]] == 0 else 0, c[2], c[3], c[4]))
+    return np.array(out, dtype=np.int32).reshape(-1, 5)
+
+
+def attn_bwd_item(q, k, v, dout, lse, dsum, cu_seqlens, scale: float, q_begin: int, q_end: int, kv_begin: int,
+                  kv_end: int):
+    """Backward contribution of ONE work item (rows [q_begin,q_end) x keys [kv_begin,kv_end), document AND causal
+    mask), given the row statistics of the COMPLETE forward: lse [N,Hq] and dsum = rowsum(dO*O) [N,Hq].
+      P = exp(scale q.k - LSE) on visible pairs; dP = dO v^T; dS = P (dP - D);
+      dQ_rows = scale dS k;  dK_keys = scale dS^T q (summed over the q-heads of a group);  dV_keys = P^T dO.
+    Returns (dq [q_end-q_begin,Hq,d], dk, dv [kv_end-kv_begin,Hkv,d]) in fp64.  Plain matrix form (small inputs).
+    Pinned by: the sum over all items of a plan equals attn_bwd_dq / attn_bwd_dkv (tests/test_executor_gloo.py)."""
+    q = np.asarray(q, np.float64); k = np.asarray(k, np.float64); v = np.asarray(v, np.float64)
+    dout = np.asarray(dout, np.float64)
+    cu = np.asarray(cu_seqlens)
+    N, Hq, d = q.shape
+    Hkv = k.shape[1]
+    g = Hq // Hkv
+    rows = np.arange(q_begin, q_end); keys = np.arange(kv_begin, kv_end)
+    doc_r = np.searchsorted(cu, rows, side="right") - 1
+    doc_k = np.searchsorted(cu, keys, side="right") - 1
+    vis = (doc_r[:, None] == doc_k[None, :]) & (keys[None, :] <= rows[:, None])
+    dq = np.zeros((len(rows), Hq, d)); dk = np.zeros((len(keys), Hkv, d)); dv = np.zeros((len(keys), Hkv, d))
+    for h in range(Hq):
+        hk = h // g
+        S = scale * q[rows, h] @ k[keys, hk].T
+        P = np.where(vis, np.exp(S - lse[rows, h][:, None]), 0.0)
+        dP = dout[rows, h] @ v[keys, hk].T
+        dS = P * (dP - dsum[rows, h][:, None])
+        dq[:, h] = scale * dS @ k[keys, hk]
+        dk[:, hk] += scale * dS.T @ q[rows, h]
+        dv[:, hk] += P.T @ dout[rows, h]
+    return dq, dk, dv

@@ -34,6 +34,7 @@ SIGNATURES = {
     "sap_plan_fwd_tiles": (ctypes.c_int64, [vp]),
     "sap_plan_schedule": (ctypes.c_int, [vp, ctypes.c_int32, vp, c_i32p]),
     "sap_plan_codegen": (ctypes.c_int32, [vp, vp, ctypes.c_int32, vp, ctypes.c_int32]),
+    "sap_plan_codegen_bwd": (ctypes.c_int32, [vp, vp, ctypes.c_int32, vp, ctypes.c_int32]),
     "sap_plan_upload": (ctypes.c_int, [vp]),
     "sap_workspace_bytes": (ctypes.c_size_t, [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
     "sap_attn_fwd": (ctypes.c_int, [vp, vp, vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int,

@@ -13,7 +13,7 @@ SAP_MASK_SKIP, SAP_MASK_FULL, SAP_MASK_DIAG = 0, 1, 2
 SAP_PASS_FWD, SAP_PASS_BWD = 0, 1
 SAP_SCHED_RING, SAP_SCHED_BALANCED = 0, 1
 SAP_OP_SEND, SAP_OP_RECV, SAP_OP_COMPUTING, SAP_OP_COPY = 0, 1, 2, 3
-SAP_T_Q, SAP_T_KV, SAP_T_O = 0, 1, 2
+SAP_T_Q, SAP_T_KV, SAP_T_O, SAP_T_DO, SAP_T_DQ, SAP_T_DKV = 0, 1, 2, 3, 4, 5
 
 
 class SapError(RuntimeError):
@@ -114,15 +114,17 @@ class Plan:
                                             ctypes.byref(n_stages)), "sap_plan_schedule")
         return slots[:self.n_items], int(n_stages.value)
 
-    def codegen(self, slots: np.ndarray, rank: int) -> np.ndarray:
-        """Jitted code generation: int32 [n_codes, 5] = (stage, opcode, tensor, peer, item) of `rank` (sap_code_t)."""
+    def codegen(self, slots: np.ndarray, rank: int, backward: bool = False) -> np.ndarray:
+        """Jitted code generation: int32 [n_codes, 5] = (stage, opcode, tensor, peer, item) of `rank` (sap_code_t),
+        for the forward (sap_plan_codegen) or the backward pass (sap_plan_codegen_bwd)."""
         L = _lib.lib()
+        fn = L.sap_plan_codegen_bwd if backward else L.sap_plan_codegen
         sl = np.ascontiguousarray(slots, dtype=np.int32)
-        n = int(L.sap_plan_codegen(self._h, sl.ctypes.data_as(ctypes.c_void_p), int(rank), None, 0))
+        n = int(fn(self._h, sl.ctypes.data_as(ctypes.c_void_p), int(rank), None, 0))
         if n < 0:
             raise SapError(-n, "sap_plan_codegen")
         codes = np.zeros((max(n, 1), 5), dtype=np.int32)
-        L.sap_plan_codegen(self._h, sl.ctypes.data_as(ctypes.c_void_p), int(rank), codes.ctypes.data_as(ctypes.c_void_p), n)
+        fn(self._h, sl.ctypes.data_as(ctypes.c_void_p), int(rank), codes.ctypes.data_as(ctypes.c_void_p), n)
         return codes[:n]
 
     def upload(self):

@@ -272,6 +272,22 @@ int sap_plan_schedule(const sap_plan_t* p, int32_t policy, sap_slot_t* slots, in
   return SAP_OK;
 }
 
+// order inside a rank's list: stage; SEND / RECV by (opcode, tensor, peer, item), COMPUTING, COPY by (tensor, peer, item)
+static int32_t emit_codes(std::vector<sap_code_t>& out, sap_code_t* codes, int32_t cap) {
+  auto phase = [](const sap_code_t& c) { return c.opcode <= SAP_OP_RECV ? 0 : (c.opcode == SAP_OP_COMPUTING ? 1 : 2); };
+  std::stable_sort(out.begin(), out.end(), [&](const sap_code_t& a, const sap_code_t& b) {
+    if (a.stage != b.stage) return a.stage < b.stage;
+    if (phase(a) != phase(b)) return phase(a) < phase(b);
+    if (phase(a) == 0 && a.opcode != b.opcode) return a.opcode < b.opcode;
+    if (a.tensor != b.tensor) return a.tensor < b.tensor;
+    if (a.peer != b.peer) return a.peer < b.peer;
+    return a.item < b.item;
+  });
+  const int32_t n = (int32_t)out.size();
+  for (int32_t c = 0; c < n && c < cap; ++c) codes[c] = out[c];
+  return n;
+}
+
 int32_t sap_plan_codegen(const sap_plan_t* p, const sap_slot_t* slots, int32_t rank, sap_code_t* codes, int32_t cap) {
   if (!p || !slots || rank < 0 || rank >= p->n_chunks || cap < 0 || (cap > 0 && !codes)) return -SAP_ERR_INVALID_ARG;
   const int32_t n_items = (int32_t)p->items.size();
@@ -292,18 +308,33 @@ int32_t sap_plan_codegen(const sap_plan_t* p, const sap_slot_t* slots, int32_t r
       if (rank == i) { out.push_back({st + 1, SAP_OP_RECV, SAP_T_O, j, x}); out.push_back({st + 1, SAP_OP_COPY, SAP_T_O, j, x}); }
     }
   }
-  auto phase = [](const sap_code_t& c) { return c.opcode <= SAP_OP_RECV ? 0 : (c.opcode == SAP_OP_COMPUTING ? 1 : 2); };
-  std::stable_sort(out.begin(), out.end(), [&](const sap_code_t& a, const sap_code_t& b) {
-    if (a.stage != b.stage) return a.stage < b.stage;
-    if (phase(a) != phase(b)) return phase(a) < phase(b);
-    if (phase(a) == 0 && a.opcode != b.opcode) return a.opcode < b.opcode;
-    if (a.tensor != b.tensor) return a.tensor < b.tensor;
-    if (a.peer != b.peer) return a.peer < b.peer;
-    return a.item < b.item;
-  });
-  const int32_t n = (int32_t)out.size();
-  for (int32_t c = 0; c < n && c < cap; ++c) codes[c] = out[c];
-  return n;
+  return emit_codes(out, codes, cap);
+}
+
+int32_t sap_plan_codegen_bwd(const sap_plan_t* p, const sap_slot_t* slots, int32_t rank, sap_code_t* codes, int32_t cap) {
+  if (!p || !slots || rank < 0 || rank >= p->n_chunks || cap < 0 || (cap > 0 && !codes)) return -SAP_ERR_INVALID_ARG;
+  const int32_t n_items = (int32_t)p->items.size();
+  std::vector<sap_code_t> out;
+  auto transfer = [&](int32_t stage, int32_t tensor, int32_t src, int32_t dst, int32_t x) {
+    if (rank == src) out.push_back({stage, SAP_OP_SEND, tensor, dst, x});
+    if (rank == dst) { out.push_back({stage, SAP_OP_RECV, tensor, src, x}); out.push_back({stage, SAP_OP_COPY, tensor, src, x}); }
+  };
+  for (int32_t x = 0; x < n_items; ++x) {
+    const sap_item_t& im = p->items[x];
+    const int32_t i = im.q_chunk, j = im.kv_chunk, R = slots[x].rank, st = slots[x].stage;
+    if (R != i && R != j) return -SAP_ERR_INVALID_ARG;
+    if (R == rank) out.push_back({st, SAP_OP_COMPUTING, -1, -1, x});
+    if (i == j) continue;
+    if (R == i) {  // K/V_j travels j -> i, the dK/dV contribution travels back
+      transfer(st - 1, SAP_T_KV, j, i, x);
+      transfer(st + 1, SAP_T_DKV, i, j, x);
+    } else {       // Q_i and dO_i (with LSE, D) travel i -> j, the dQ contribution travels back
+      transfer(st - 1, SAP_T_Q, i, j, x);
+      transfer(st - 1, SAP_T_DO, i, j, x);
+      transfer(st + 1, SAP_T_DQ, j, i, x);
+    }
+  }
+  return emit_codes(out, codes, cap);
 }
 
 const char* sap_strerror(int status) {

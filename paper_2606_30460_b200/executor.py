@@ -17,7 +17,8 @@ from typing import Callable
 
 import numpy as np
 
-from .api import Plan, SAP_OP_COMPUTING, SAP_OP_COPY, SAP_OP_RECV, SAP_OP_SEND, SAP_T_KV, SAP_T_O, SAP_T_Q
+from .api import (Plan, SAP_OP_COMPUTING, SAP_OP_COPY, SAP_OP_RECV, SAP_OP_SEND, SAP_T_DKV, SAP_T_DO, SAP_T_DQ, SAP_T_KV,
+                  SAP_T_O, SAP_T_Q)
 
 
 def sap_execute_fwd(q_shard, kv_shard, plan: Plan, slots: np.ndarray, rank: int, partial_fn: Callable,
@@ -72,3 +73,63 @@ def sap_execute_fwd(q_shard, kv_shard, plan: Plan, slots: np.ndarray, rank: int,
     assert not q_buf and not kv_buf and not results, "every transferred tensor was consumed"
     return acc if acc is not None else (None, None)
 
+
+
+def sap_execute_bwd(q_shard, do_pack, kv_shard, plan: Plan, slots: np.ndarray, rank: int, bwd_fn: Callable, group=None):
+    """Replays rank `rank`'s backward code list (sap_plan_codegen_bwd).  q_shard [n,Hq,d]; do_pack: this rank's dO
+    rows with their LSE and D packed in one tensor (it travels as the `do` tensor of Table 1); kv_shard [2,n,Hkv,d].
+    bwd_fn(item, q_shard, do_pack, kv_shard) -> (dq [n,Hq,d], dkv [2,n,Hkv,d]) : the item's contributions to the rows
+    of chunk q_chunk(item) and to the keys of chunk kv_chunk(item), as tensors torch.distributed can send.
+    Returns this rank's (dq, dkv): own contributions plus everything the COPY codes added."""
+    import torch
+    import torch.distributed as dist
+
+    codes = plan.codegen(slots, rank, backward=True)
+    items = plan.items
+    dq_acc, dkv_acc = None, None
+    bufs, results = {}, {}                      # (tensor, item) -> received operand; (tensor, item) -> contribution to send
+    add = lambda acc, t: t.clone() if acc is None else acc + t
+    for st in sorted(set(int(c[0]) for c in codes)):
+        mine = [tuple(int(v) for v in c) for c in codes if int(c[0]) == st]
+        ops, recv = [], {}
+        for _, op, tensor, peer, item in mine:
+            if op == SAP_OP_SEND:
+                payload = {SAP_T_Q: q_shard, SAP_T_DO: do_pack, SAP_T_KV: kv_shard}.get(tensor)
+                if payload is None:
+                    payload = results.pop((tensor, item))
+                ops.append(dist.P2POp(dist.isend, payload.contiguous(), peer, group))
+            elif op == SAP_OP_RECV:
+                like = {SAP_T_Q: q_shard, SAP_T_DO: do_pack, SAP_T_KV: kv_shard, SAP_T_DQ: q_shard, SAP_T_DKV: kv_shard}[tensor]
+                recv[(tensor, item)] = torch.empty_like(like)
+                ops.append(dist.P2POp(dist.irecv, recv[(tensor, item)], peer, group))
+        reqs = dist.batch_isend_irecv(ops) if ops else []
+        for _, op, tensor, peer, item in mine:
+            if op != SAP_OP_COMPUTING:
+                continue
+            i, j = int(items[item, 0]), int(items[item, 1])
+            qs = q_shard if i == rank else bufs.pop((SAP_T_Q, item))
+            dos = do_pack if i == rank else bufs.pop((SAP_T_DO, item))
+            kv = kv_shard if j == rank else bufs.pop((SAP_T_KV, item))
+            dq, dkv = bwd_fn(item, qs, dos, kv)
+            if i == rank:
+                dq_acc = add(dq_acc, dq)
+            else:
+                results[(SAP_T_DQ, item)] = dq      # travels back to the rank of the rows one stage later
+            if j == rank:
+                dkv_acc = add(dkv_acc, dkv)
+            else:
+                results[(SAP_T_DKV, item)] = dkv    # travels back to the rank of the keys one stage later
+        for r in reqs:
+            r.wait()
+        for _, op, tensor, peer, item in mine:
+            if op != SAP_OP_COPY:
+                continue
+            buf = recv.pop((tensor, item))
+            if tensor == SAP_T_DQ:
+                dq_acc = add(dq_acc, buf)
+            elif tensor == SAP_T_DKV:
+                dkv_acc = add(dkv_acc, buf)
+            else:
+                bufs[(tensor, item)] = buf
+    assert not bufs and not results, "every transferred tensor was consumed"
+    return dq_acc, dkv_acc
