@@ -228,6 +228,10 @@ int64_t sap_launch_count(void);
  * q-heads of one GQA group per CTA, sharing the K/V tiles) whenever Hq/Hkv is even, the one-head kernel otherwise;
  * 1: always the one-head kernel.  Process-wide; returns the previous value. */
 int sap_debug_set_fwd_form(int form);
+/* Diagnostic: which fused backward main kernel runs at head_dim 128.  0 (default): the CTA-pair kernel (tcgen05
+ * cta_group::2 over 256-key pair-tiles); 1: the one-CTA kernel (always used at head_dim 64).  Process-wide; returns the
+ * previous value. */
+int sap_debug_set_bwd_form(int form);
 /* Diagnostic: which kernels sap_attn_bwd launches, so each can be timed alone and the two forms of the main
  * pass compared.  Bits: 1 = D pre-pass, 8 = fused main kernel (dK, dV, fp32 dQ accumulator; 5 GEMMs per tile
  * pair; zeroes the accumulator first), 16 = dQ post pass (bf16(scale * accumulator)); 2 = split dK/dV kernel,

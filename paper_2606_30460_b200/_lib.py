@@ -58,6 +58,7 @@ SIGNATURES = {
     "sap_launch_count": (ctypes.c_int64, []),
     "sap_debug_set_bwd_stages": (ctypes.c_int, [ctypes.c_int]),
     "sap_debug_set_fwd_form": (ctypes.c_int, [ctypes.c_int]),
+    "sap_debug_set_bwd_form": (ctypes.c_int, [ctypes.c_int]),
 }
 
 _lib = None

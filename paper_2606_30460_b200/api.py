@@ -237,6 +237,11 @@ def sap_debug_set_fwd_form(form: int) -> int:
     return int(_lib.lib().sap_debug_set_fwd_form(int(form)))
 
 
+def sap_debug_set_bwd_form(form: int) -> int:
+    """Diagnostic: 0 = CTA-pair fused backward at head_dim 128 (default), 1 = always the one-CTA fused kernel."""
+    return int(_lib.lib().sap_debug_set_bwd_form(int(form)))
+
+
 # ---- per-rank launches (SURVEY 8(f) NEXT-1): the same kernels restricted to the chunks one rank owns ----------------
 def sap_attn_fwd_chunks(q, k, v, cu_seqlens_dev, plan: Plan, q_chunk_begin: int, q_chunk_end: int, out, lse,
                         softmax_scale: Optional[float] = None, stream=None):

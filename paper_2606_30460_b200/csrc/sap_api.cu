@@ -7,6 +7,7 @@
 #include "sap_fwd_pair.cuh"
 #include "sap_bwd.cuh"
 #include "sap_bwd_fused.cuh"
+#include "sap_bwd_pair.cuh"
 #include "sap_merge.cuh"
 
 namespace sap {
@@ -19,7 +20,8 @@ static inline size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
 thread_local int g_last_cuda_error = 0;
 std::atomic<int64_t> g_launch_count{0};
 std::atomic<int> g_bwd_stages{kBwdDefaultStages};
-std::atomic<int> g_fwd_form{0};  // 0: pair kernel when Hq/Hkv is even, 1: always the one-head kernel (diagnostic)
+std::atomic<int> g_fwd_form{0};
+std::atomic<int> g_bwd_form{0};  // 0: CTA-pair fused kernel for head_dim 128, 1: always the one-CTA fused kernel (diagnostic)  // 0: pair kernel when Hq/Hkv is even, 1: always the one-head kernel (diagnostic)
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -122,6 +124,44 @@ static int launch_fwd(const DevProgram& prog, const void* q, const void* k, cons
   return SAP_OK;
 }
 
+// a6: the fused main kernel over a KV-stationary program.  head_dim 128 runs on CTA pairs over the 256-key program
+// `prog2`, head_dim 64 (and the diagnostic form) on single CTAs over the 128-key program `prog1`.
+template <int D>
+static int launch_bwd_main(const DevProgram& prog1, const DevProgram& prog2, const void* dout, const void* q, const void* k,
+                           const void* v, const float* lse, const int32_t* cu, const sap_plan_t* plan, void* dk, void* dv,
+                           int Hq, int Hkv, float scale, const float* dsum, float* dq_acc, cudaStream_t stream) {
+  const int64_t N = plan->n_tokens;
+  CUtensorMap mq64, mdo64, mk128, mv128;
+  int rc;
+  if ((rc = make_tile_map(&mq64, q, N, (int64_t)Hq * D, kBwdN)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mdo64, dout, N, (int64_t)Hq * D, kBwdN)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mk128, k, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
+  if ((rc = make_tile_map(&mv128, v, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
+  static bool attr_set = false;
+  if (!attr_set) {
+    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_fused_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FusedSmem<D>::kTotal));
+    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PairSmem::kTotal));
+    attr_set = true;
+  }
+  if (D == 128 && g_bwd_form.load() == 0) {
+    if (prog2.n_tiles == 0) return SAP_OK;
+    CUtensorMap mq32, mdo32;
+    if ((rc = make_tile_map(&mq32, q, N, (int64_t)Hq * D, 32)) != SAP_OK) return rc;
+    if ((rc = make_tile_map(&mdo32, dout, N, (int64_t)Hq * D, 32)) != SAP_OK) return rc;
+    sap_bwd_pair_kernel<<<2u * static_cast<unsigned>(prog2.n_tiles) * Hkv, kPairThreads, PairSmem::kTotal, stream>>>(
+        mq32, mdo32, mq64, mdo64, mk128, mv128, prog2.tiles, prog2.segs, cu, plan->n_docs, lse, dsum, dq_acc,
+        static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
+  } else {
+    if (prog1.n_tiles == 0) return SAP_OK;
+    sap_bwd_fused_kernel<D><<<static_cast<unsigned>(prog1.n_tiles) * Hkv, kFusedThreads, FusedSmem<D>::kTotal, stream>>>(
+        mq64, mdo64, mk128, mv128, prog1.tiles, prog1.segs, cu, plan->n_docs, lse, dsum, dq_acc,
+        static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
+  }
+  g_launch_count.fetch_add(1);
+  SAP_CUDA_CHECK(cudaGetLastError());
+  return SAP_OK;
+}
+
 template <int D>
 static int launch_bwd(const PlanDevice* pd, const void* dout, const void* q, const void* k, const void* v,
                       const void* out, const float* lse, const int32_t* cu, const sap_plan_t* plan, void* dq, void* dk,
@@ -152,17 +192,12 @@ static int launch_bwd(const PlanDevice* pd, const void* dout, const void* q, con
   if (!attr_set) {
     SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_dq_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, DqSmem<D>::kTotal));
     SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_dkv_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, DkvSmem<D>::kTotal));
-    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_fused_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FusedSmem<D>::kTotal));
     attr_set = true;
   }
   // a6 fused: dK, dV and the fp32 dQ accumulator in one pass (5 GEMMs per tile pair)
   if (stages & 8) {
     SAP_CUDA_CHECK(cudaMemsetAsync(dq_acc, 0, static_cast<size_t>(N) * Hq * D * sizeof(float), stream));
-    sap_bwd_fused_kernel<D><<<static_cast<unsigned>(pd->kv.n_tiles) * Hkv, kFusedThreads, FusedSmem<D>::kTotal, stream>>>(
-        mq64, mdo64, mk128, mv128, pd->kv.tiles, pd->kv.segs, cu, plan->n_docs, lse, dsum, dq_acc,
-        static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
-    g_launch_count.fetch_add(1);
-    SAP_CUDA_CHECK(cudaGetLastError());
+    if ((rc = launch_bwd_main<D>(pd->kv, pd->kv2, dout, q, k, v, lse, cu, plan, dk, dv, Hq, Hkv, scale, dsum, dq_acc, stream)) != SAP_OK) return rc;
   }
   // a7: dq = bf16(scale * dq_acc)
   if (stages & 16) {
@@ -205,31 +240,6 @@ static int launch_bwd_begin(const void* dout, const void* out, int64_t N, int Hq
   return SAP_OK;
 }
 
-template <int D>
-static int launch_bwd_fused_program(const DevProgram& prog, const void* dout, const void* q, const void* k, const void* v,
-                                    const float* lse, const int32_t* cu, const sap_plan_t* plan, void* dk, void* dv, int Hq,
-                                    int Hkv, float scale, const float* dsum, float* dq_acc, cudaStream_t stream) {
-  const int64_t N = plan->n_tokens;
-  CUtensorMap mq64, mdo64, mk128, mv128;
-  int rc;
-  if ((rc = make_tile_map(&mq64, q, N, (int64_t)Hq * D, kBwdN)) != SAP_OK) return rc;
-  if ((rc = make_tile_map(&mdo64, dout, N, (int64_t)Hq * D, kBwdN)) != SAP_OK) return rc;
-  if ((rc = make_tile_map(&mk128, k, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
-  if ((rc = make_tile_map(&mv128, v, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
-  static bool attr_set = false;
-  if (!attr_set) {
-    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_fused_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FusedSmem<D>::kTotal));
-    attr_set = true;
-  }
-  if (prog.n_tiles == 0) return SAP_OK;
-  sap_bwd_fused_kernel<D><<<static_cast<unsigned>(prog.n_tiles) * Hkv, kFusedThreads, FusedSmem<D>::kTotal, stream>>>(
-      mq64, mdo64, mk128, mv128, prog.tiles, prog.segs, cu, plan->n_docs, lse, dsum, dq_acc,
-      static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
-  g_launch_count.fetch_add(1);
-  SAP_CUDA_CHECK(cudaGetLastError());
-  return SAP_OK;
-}
-
 static int launch_bwd_end(const float* dq_acc, void* dq, int Hq, int d, int64_t t0, int64_t nt, float scale, cudaStream_t stream) {
   const int64_t n8 = nt * Hq * d / 8;
   if (n8 == 0) return SAP_OK;
@@ -243,15 +253,17 @@ static int launch_bwd_end(const float* dq_acc, void* dq, int Hq, int d, int64_t 
 }
 
 // item-range (forward) or kv-chunk-range (backward) restricted programs, built once per range and kept with the plan
-static int get_chunk_program(sap_plan_t* plan, bool kv, int32_t c_begin, int32_t c_end, DevProgram* out) {
+// kind: 0 Q-stationary program of q-chunks, 1 KV-stationary of kv-chunks (128-key tiles), 2 the same with 256-key pair-tiles
+static int get_chunk_program(sap_plan_t* plan, int kind, int32_t c_begin, int32_t c_end, DevProgram* out) {
   PlanDevice* pd = static_cast<PlanDevice*>(plan->dev_state);
   std::lock_guard<std::mutex> lock(plan->mu);
-  auto& cache = kv ? pd->kv_chunks : pd->q_chunks;
+  const bool kv = kind != 0;
+  auto& cache = kind == 2 ? pd->kv2_chunks : (kind == 1 ? pd->kv_chunks : pd->q_chunks);
   auto key = std::make_pair(c_begin, c_end);
   auto itp = cache.find(key);
   if (itp == cache.end()) {
     TileProgram host;
-    if (kv) build_kv_program(*plan, host, c_begin, c_end);
+    if (kv) build_kv_program(*plan, host, c_begin, c_end, kind == 2 ? 2 * kTile : kTile);
     else build_q_program(*plan, plan->chunk_offsets[c_begin], plan->chunk_offsets[c_end], host, /*drop_empty=*/true);
     DevProgram dp;
     int rc = upload_program(host, dp);
@@ -278,8 +290,14 @@ int64_t sap_launch_count(void) { return g_launch_count.load(); }
 int sap_debug_read_trace(unsigned long long* host_out) {
   return (int)cudaMemcpyFromSymbol(host_out, g_sap_trace, sizeof(unsigned long long) * 128 * 64);
 }
+int sap_debug_clear_trace(void) {   // zero everything; slots 21 / 53 (atomicMin stamps) start at the maximum
+  static unsigned long long h[128 * 64];
+  for (int i = 0; i < 128; ++i) for (int s2 = 0; s2 < 64; ++s2) h[i * 64 + s2] = (s2 == 21 || s2 == 53) ? ~0ull : 0ull;
+  return (int)cudaMemcpyToSymbol(g_sap_trace, h, sizeof(h));
+}
 #endif
 int sap_debug_set_fwd_form(int form) { return g_fwd_form.exchange(form ? 1 : 0); }
+int sap_debug_set_bwd_form(int form) { return g_bwd_form.exchange(form ? 1 : 0); }
 int sap_debug_set_bwd_stages(int mask) { return g_bwd_stages.exchange(mask < 0 ? kBwdDefaultStages : (mask & 31)); }
 
 int sap_plan_upload(sap_plan_t* plan) {
@@ -293,6 +311,7 @@ int sap_plan_upload(sap_plan_t* plan) {
   SAP_CUDA_CHECK(cudaGetDevice(&pd->device));
   if ((rc = upload_program(plan->fwd, pd->fwd)) != SAP_OK) return rc;
   if ((rc = upload_program(plan->kv, pd->kv)) != SAP_OK) return rc;
+  if ((rc = upload_program(plan->kv2, pd->kv2)) != SAP_OK) return rc;
   pd->uploaded = true;
   return SAP_OK;
 }
@@ -303,9 +322,11 @@ void sap_plan_destroy(sap_plan_t* plan) {
   if (pd) {
     free_program(pd->fwd);
     free_program(pd->kv);
+    free_program(pd->kv2);
     for (auto& kv : pd->partial) free_program(kv.second);
     for (auto& kv : pd->q_chunks) free_program(kv.second);
     for (auto& kv : pd->kv_chunks) free_program(kv.second);
+    for (auto& kv : pd->kv2_chunks) free_program(kv.second);
     delete pd;
   }
   delete plan;
@@ -426,7 +447,7 @@ int sap_attn_fwd_chunks(const void* q, const void* k, const void* v, const int32
   if ((rc = sap_plan_upload(plan)) != SAP_OK) return rc;
   if (q_chunk_begin == q_chunk_end) return SAP_OK;
   DevProgram prog;
-  if ((rc = get_chunk_program(plan, false, q_chunk_begin, q_chunk_end, &prog)) != SAP_OK) return rc;
+  if ((rc = get_chunk_program(plan, 0, q_chunk_begin, q_chunk_end, &prog)) != SAP_OK) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (head_dim == 128)
     return launch_fwd<128, false>(prog, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st);
@@ -472,14 +493,15 @@ int sap_attn_bwd_chunks(const void* dout, const void* q, const void* k, const vo
   if ((rc = bwd_ws(plan, n_q_heads, n_kv_heads, head_dim, workspace, workspace_bytes, &dsum, &dq_acc)) != SAP_OK) return rc;
   if ((rc = sap_plan_upload(plan)) != SAP_OK) return rc;
   if (kv_chunk_begin == kv_chunk_end) return SAP_OK;
+  const bool pair = head_dim == 128 && g_bwd_form.load() == 0;
   DevProgram prog;
-  if ((rc = get_chunk_program(plan, true, kv_chunk_begin, kv_chunk_end, &prog)) != SAP_OK) return rc;
+  if ((rc = get_chunk_program(plan, pair ? 2 : 1, kv_chunk_begin, kv_chunk_end, &prog)) != SAP_OK) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (head_dim == 128)
-    return launch_bwd_fused_program<128>(prog, dout, q, k, v, lse, cu_seqlens_dev, plan, dk, dv, n_q_heads, n_kv_heads,
-                                         softmax_scale, dsum, dq_acc, st);
-  return launch_bwd_fused_program<64>(prog, dout, q, k, v, lse, cu_seqlens_dev, plan, dk, dv, n_q_heads, n_kv_heads,
-                                      softmax_scale, dsum, dq_acc, st);
+    return launch_bwd_main<128>(prog, prog, dout, q, k, v, lse, cu_seqlens_dev, plan, dk, dv, n_q_heads, n_kv_heads,
+                                softmax_scale, dsum, dq_acc, st);
+  return launch_bwd_main<64>(prog, prog, dout, q, k, v, lse, cu_seqlens_dev, plan, dk, dv, n_q_heads, n_kv_heads,
+                             softmax_scale, dsum, dq_acc, st);
 }
 
 int sap_attn_bwd_end(sap_plan_t* plan, int32_t q_chunk_begin, int32_t q_chunk_end, void* dq, int n_q_heads, int n_kv_heads,

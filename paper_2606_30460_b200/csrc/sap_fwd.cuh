@@ -21,8 +21,15 @@ namespace sap {
 #ifdef SAP_TRACE  // instrumented build only (never the shipped library): SM cycle stamps of one CTA
 __device__ unsigned long long g_sap_trace[128 * 64];
 #define SAP_STAMP(iter, slot) do { if (blockIdx.x == 0 && (iter) < 128) g_sap_trace[(iter) * 64 + (slot)] = clock64(); } while (0)
+// CTA pairs: slots [0,32) of the leader (block 0), [32,64) of its peer (block 1); the two SMs' clocks are not aligned
+#define SAP_STAMP2(iter, slot) do { if (blockIdx.x < 2 && (iter) < 128) g_sap_trace[(iter) * 64 + 32 * blockIdx.x + (slot)] = clock64(); } while (0)
+#define SAP_STAMP_MAX(iter, slot) do { if (blockIdx.x < 2 && (iter) < 128) atomicMax(&g_sap_trace[(iter) * 64 + 32 * blockIdx.x + (slot)], (unsigned long long)clock64()); } while (0)
+#define SAP_STAMP_MIN(iter, slot) do { if (blockIdx.x < 2 && (iter) < 128) atomicMin(&g_sap_trace[(iter) * 64 + 32 * blockIdx.x + (slot)], (unsigned long long)clock64()); } while (0)
 #else
 #define SAP_STAMP(iter, slot) do { } while (0)
+#define SAP_STAMP_MAX(iter, slot) do { } while (0)
+#define SAP_STAMP_MIN(iter, slot) do { } while (0)
+#define SAP_STAMP2(iter, slot) do { } while (0)
 #endif
 
 constexpr int kFwdThreads = 256;

@@ -32,9 +32,9 @@ struct DevProgram {
 struct PlanDevice {
   bool uploaded = false;
   int device = -1;
-  DevProgram fwd, kv;
+  DevProgram fwd, kv, kv2;
   std::map<std::pair<int32_t, int32_t>, DevProgram> partial;  // item-range-restricted Q programs
-  std::map<std::pair<int32_t, int32_t>, DevProgram> q_chunks, kv_chunks;  // chunk-range-restricted programs (per-rank launches)
+  std::map<std::pair<int32_t, int32_t>, DevProgram> q_chunks, kv_chunks, kv2_chunks;  // chunk-range-restricted programs (per-rank launches)
 };
 
 int check_device_is_sm100();

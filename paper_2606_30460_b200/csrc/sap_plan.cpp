@@ -75,17 +75,18 @@ void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, Ti
   out.tiles.swap(sorted);
 }
 
-void build_kv_program(const sap_plan& p, TileProgram& out, int32_t chunk_begin, int32_t chunk_end) {
+void build_kv_program(const sap_plan& p, TileProgram& out, int32_t chunk_begin, int32_t chunk_end, int32_t tile_rows) {
   out.tiles.clear();
   out.segs.clear();
   out.streamed_tiles = 0;
   const int64_t n = p.chunk_len, N = p.n_tokens;
   std::vector<int64_t> work;
-  // K/V tiles are globally 128-aligned (they must match the key tiles the forward kernel streams only in
-  // coverage, not in alignment); a tile that straddles two kv-chunks gets segments from both.
+  // K/V tiles of `tile_rows` keys (128: one CTA; 256: a CTA pair) counted from the first key of the range (they must
+  // match the key tiles the forward kernel streams only in coverage, not in alignment); a tile that straddles two
+  // kv-chunks gets segments from both.
   const int64_t k_begin = (int64_t)chunk_begin * n, k_end = chunk_end < 0 ? N : (int64_t)chunk_end * n;  // 128-aligned when restricted
-  for (int64_t c0 = k_begin; c0 < k_end; c0 += kTile) {
-    const int64_t c1 = std::min<int64_t>(c0 + kTile, k_end);
+  for (int64_t c0 = k_begin; c0 < k_end; c0 += tile_rows) {
+    const int64_t c1 = std::min<int64_t>(c0 + tile_rows, k_end);
     TileDesc td;
     td.row0 = (int32_t)c0;
     td.rows = (int32_t)(c1 - c0);
@@ -189,6 +190,7 @@ int sap_plan_create(const int32_t* cu, int32_t n_docs, int32_t n_chunks, sap_pla
   }
   build_q_program(*p, 0, (int32_t)p->items.size(), p->fwd);
   build_kv_program(*p, p->kv);
+  build_kv_program(*p, p->kv2, 0, -1, 2 * kTile);
   *out = p;
   return SAP_OK;
 }
