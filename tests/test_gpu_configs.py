@@ -22,7 +22,7 @@ import torch
 import paper_2606_30460_b200 as sap
 from oracle import oracle
 from paper_2606_30460_b200.workloads import make_qkv, make_workload
-from parity import check_close, check_lse, to_np
+from parity import check_close, check_lse, to_np, row_scale, col_scale
 
 pytestmark = pytest.mark.gpu
 
@@ -87,16 +87,18 @@ def test_full_size_config_sampled_against_oracle(cfg):
     rows = sample_rows(w, n_random, rng)
     o_ref, l_ref = oracle.attn_fwd(*args, w.cu_seqlens, w.softmax_scale, rows=rows)
     rows_t = torch.from_numpy(rows).cuda()
-    check_close(to_np(out[rows_t][:, q_sel]), o_ref, f"cfg{cfg} out[{len(rows)} rows]")
+    nk = row_scale(w.cu_seqlens, rows)
+    check_close(to_np(out[rows_t][:, q_sel]), o_ref, f"cfg{cfg} out[{len(rows)} rows]", nk)
     check_lse(to_np(lse[q_sel][:, rows_t]).T, l_ref, f"cfg{cfg} lse")
     dq_ref = oracle.attn_bwd_dq(*args, dos, w.cu_seqlens, w.softmax_scale, rows=rows)
-    check_close(to_np(dq[rows_t][:, q_sel]), dq_ref, f"cfg{cfg} dq[{len(rows)} rows]")
+    check_close(to_np(dq[rows_t][:, q_sel]), dq_ref, f"cfg{cfg} dq[{len(rows)} rows]", nk)
 
     cols = sample_cols(w, rng)
     dk_ref, dv_ref = oracle.attn_bwd_dkv(*args, dos, w.cu_seqlens, w.softmax_scale, cols=cols)
     cols_t = torch.from_numpy(cols).cuda()
-    check_close(to_np(dk[cols_t][:, list(kv_sel)]), dk_ref, f"cfg{cfg} dk[{len(cols)} cols]")
-    check_close(to_np(dv[cols_t][:, list(kv_sel)]), dv_ref, f"cfg{cfg} dv[{len(cols)} cols]")
+    nr = col_scale(w.cu_seqlens, cols)
+    check_close(to_np(dk[cols_t][:, list(kv_sel)]), dk_ref, f"cfg{cfg} dk[{len(cols)} cols]", nr)
+    check_close(to_np(dv[cols_t][:, list(kv_sel)]), dv_ref, f"cfg{cfg} dv[{len(cols)} cols]", nr)
 
     # sparse dO: every key column against the live rows
     live = np.unique(np.concatenate([rng.integers(0, N, size=n_live), rows[:: max(1, len(rows) // 48)]]))
@@ -113,7 +115,7 @@ def test_full_size_config_sampled_against_oracle(cfg):
     dead = torch.ones(N, dtype=torch.bool, device="cuda"); dead[live_t] = False
     assert float(dq2[dead].abs().max()) == 0.0   # rows with dO = 0 have dQ = 0 exactly
     dq_ref2 = oracle.attn_bwd_dq(*args, dos_sp, w.cu_seqlens, w.softmax_scale, rows=live)
-    check_close(to_np(dq2[live_t][:, q_sel]), dq_ref2, f"cfg{cfg} dq, sparse dO, live rows")
+    check_close(to_np(dq2[live_t][:, q_sel]), dq_ref2, f"cfg{cfg} dq, sparse dO, live rows", row_scale(w.cu_seqlens, live))
 
 
 def test_cfg2_partials_plus_merge_equal_fused_full_size():
