@@ -16,8 +16,13 @@
  * Conventions
  *   - Every function returns an int status (0 = SAP_OK); nothing throws, nothing aborts.
  *   - "host" / "device" is stated per pointer.  Device buffers are owned by the caller; the library
- *     allocates device memory only for a plan's device mirror (sap_plan_upload) and frees it in
- *     sap_plan_destroy.  No call synchronises the device except sap_plan_upload.
+ *     allocates device memory only for a plan's device mirror (sap_plan_upload, and the range-restricted
+ *     programs of the partial / per-rank / per-item calls, built on first use of a range and uploaded on
+ *     the caller's stream) and frees it in sap_plan_destroy.  Only sap_plan_upload and sap_plan_destroy
+ *     synchronise the device; every other call is asynchronous on its stream.
+ *   - A plan's device mirror lives on one device (the current device of its first upload); every attention call takes
+ *     the caller's token count n_tokens and fails with SAP_ERR_PLAN_MISMATCH when it differs from the plan's (the kernels
+ *     index the tensors by the plan's token ranges) or when the current device is another one.
  *   - Layouts (packed "thd"): q/out/dout/dq  [N, Hq,  d] bf16, contiguous;
  *     k/v/dk/dv [N, Hkv, d] bf16, contiguous; lse [Hq, N] fp32 (natural log of the sum of
  *     exp(scale * q.k) over the visible keys); cu_seqlens int32 [D+1], cu[0] = 0, non-decreasing,
@@ -36,7 +41,7 @@
 extern "C" {
 #endif
 
-/* ---- status codes ------------------------------------------------------------------------- */
+/* ---- status codes (every call returns one; the paper's executor has no error model, this is the library's) ---- */
 enum {
   SAP_OK = 0,
   SAP_ERR_INVALID_ARG = 1,        /* null pointer, n_chunks < 1, n_docs < 1, bad range               */
@@ -46,7 +51,8 @@ enum {
   SAP_ERR_WORKSPACE_TOO_SMALL = 5,
   SAP_ERR_WRONG_ARCH = 6,         /* current device is not compute capability 10.x                    */
   SAP_ERR_CUDA = 7,               /* a CUDA runtime/driver call failed; see sap_last_cuda_error()     */
-  SAP_ERR_NO_DEVICE = 8           /* no CUDA device / driver available                                */
+  SAP_ERR_NO_DEVICE = 8,          /* no CUDA device / driver available                                */
+  SAP_ERR_PLAN_MISMATCH = 9       /* n_tokens != the plan's token count, or the plan's mirror is on another device */
 };
 
 /* ---- plan (host-side JIT planner; §3.2 Step 1, :106-:108) ------------------------- */
@@ -134,16 +140,18 @@ int32_t sap_plan_codegen(const sap_plan_t* plan, const sap_slot_t* slots, int32_
 enum { SAP_T_DO = 3, SAP_T_DQ = 4, SAP_T_DKV = 5 };
 int32_t sap_plan_codegen_bwd(const sap_plan_t* plan, const sap_slot_t* slots, int32_t rank, sap_code_t* codes, int32_t cap);
 
-/* Copy the compiled work lists to the current CUDA device (cudaMalloc + synchronous cudaMemcpy).
- * Called implicitly by the first sap_attn_* call that uses the plan; call it yourself to keep that
- * cost out of a timed region.  Idempotent, thread-safe. */
+/* Copy the compiled work lists to the current CUDA device (cudaMalloc + synchronous cudaMemcpy): the "compile" side
+ * runs "ahead of the communication and computation".  Called implicitly by the first sap_attn_* call that
+ * uses the plan; call it yourself to keep that cost out of a timed region.  Idempotent; serialised per plan by a mutex;
+ * a failed upload frees what it had allocated.  SAP_ERR_PLAN_MISMATCH if the plan is already on another device. */
 int sap_plan_upload(sap_plan_t* plan);
 
 /* ---- attention ------------------------------------------------------------------------------ */
 enum { SAP_PASS_FWD = 0, SAP_PASS_BWD = 1 };
 
 /* Bytes of caller-provided device workspace a pass needs (fwd: 0; bwd: D = rowsum(dO*O), fp32 [Hq,N], padded to
- * 256 B, followed by the fp32 dQ accumulator [N,Hq,d] the fused backward kernel reduces into). */
+ * 256 B, followed by the fp32 dQ accumulator [N,Hq,d] the fused backward kernel reduces into).  A buffer of fixed,
+ * known size that the caller allocates once: the paper's "fixed global buffer ... no memory jitter". */
 size_t sap_workspace_bytes(const sap_plan_t* plan, int n_q_heads, int n_kv_heads, int head_dim, int pass);
 
 /* Forward: for every row, attention over the visible keys, walking the row's
@@ -151,7 +159,7 @@ size_t sap_workspace_bytes(const sap_plan_t* plan, int n_q_heads, int n_kv_heads
  * q,k,v,cu_seqlens_dev: device, read.  out: device bf16 [N,Hq,d], written.  lse: device fp32 [Hq,N], written.
  * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Asynchronous. */
 int sap_attn_fwd(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev,
-                 sap_plan_t* plan, void* out, float* lse,
+                 sap_plan_t* plan, int64_t n_tokens, void* out, float* lse,
                  int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
                  void* workspace, size_t workspace_bytes, void* cuda_stream);
 
@@ -160,7 +168,7 @@ int sap_attn_fwd(const void* q, const void* k, const void* v, const int32_t* cu_
  * Rows with no visible key among those items get out = 0, lse = -inf.  Items of one q-chunk cover
  * disjoint key sets, so partials of disjoint item sets merge exactly with sap_lse_merge. */
 int sap_attn_fwd_partial(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev,
-                         sap_plan_t* plan, int32_t item_begin, int32_t item_end,
+                         sap_plan_t* plan, int64_t n_tokens, int32_t item_begin, int32_t item_end,
                          float* out_f32, float* lse,
                          int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
                          void* cuda_stream);
@@ -183,7 +191,7 @@ int sap_lse_merge(const float* o_a, const float* lse_a, const float* o_b, const 
  * sap_workspace_bytes(plan, ..., SAP_PASS_BWD) bytes.  dQ is reduced in fp32 with atomic adds, so its low
  * bits may differ from run to run (any accumulation order is correct, A-14); dK, dV are deterministic. */
 int sap_attn_bwd(const void* dout, const void* q, const void* k, const void* v, const void* out,
-                 const float* lse, const int32_t* cu_seqlens_dev, sap_plan_t* plan,
+                 const float* lse, const int32_t* cu_seqlens_dev, sap_plan_t* plan, int64_t n_tokens,
                  void* dq, void* dk, void* dv,
                  int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
                  void* workspace, size_t workspace_bytes, void* cuda_stream);
@@ -206,18 +214,50 @@ int sap_attn_bwd(const void* dout, const void* q, const void* k, const void* v, 
  *   sap_attn_bwd_end    : dq rows of q-chunks [begin, end) = bf16(scale * accumulator)
  * All asynchronous on cuda_stream; device pointers as in sap_attn_fwd / sap_attn_bwd. */
 int sap_attn_fwd_chunks(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev, sap_plan_t* plan,
-                        int32_t q_chunk_begin, int32_t q_chunk_end, void* out, float* lse,
+                        int64_t n_tokens, int32_t q_chunk_begin, int32_t q_chunk_end, void* out, float* lse,
                         int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale, void* cuda_stream);
-int sap_attn_bwd_begin(const void* dout, const void* out, sap_plan_t* plan, int32_t q_chunk_begin, int32_t q_chunk_end,
+int sap_attn_bwd_begin(const void* dout, const void* out, sap_plan_t* plan, int64_t n_tokens, int32_t q_chunk_begin, int32_t q_chunk_end,
                        int n_q_heads, int n_kv_heads, int head_dim, void* workspace, size_t workspace_bytes,
                        void* cuda_stream);
 int sap_attn_bwd_chunks(const void* dout, const void* q, const void* k, const void* v, const float* lse,
-                        const int32_t* cu_seqlens_dev, sap_plan_t* plan, int32_t kv_chunk_begin, int32_t kv_chunk_end,
+                        const int32_t* cu_seqlens_dev, sap_plan_t* plan, int64_t n_tokens, int32_t kv_chunk_begin, int32_t kv_chunk_end,
                         void* dk, void* dv, int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
                         void* workspace, size_t workspace_bytes, void* cuda_stream);
-int sap_attn_bwd_end(sap_plan_t* plan, int32_t q_chunk_begin, int32_t q_chunk_end, void* dq,
+int sap_attn_bwd_end(sap_plan_t* plan, int64_t n_tokens, int32_t q_chunk_begin, int32_t q_chunk_end, void* dq,
                      int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
                      void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---- per-item launches: the `computing` instruction of the backward pass -------------------
+ * sap_attn_bwd_items: the fused backward kernel restricted to plan items [item_begin, item_end) (Table 1, PAPER.md:85-98:
+ * one `computing` code = one item; the tensors it reads are q / do of the item's rows and kv of its keys, the ones it
+ * produces are the dq and dkv CONTRIBUTIONS of that item, :87-96).  K/V-stationary over the 256-key (head_dim 128) or
+ * 128-key tiles that intersect the items' key ranges:
+ *   dk, dv : device bf16 [N,Hkv,d]; rows of every touched tile are written with the items' contribution (zero where no
+ *            item contributes), rows of untouched tiles are left alone - pass scratch buffers and take
+ *            [kv_begin, kv_end) of each item;
+ *   dQ     : contributions are ADDED into the fp32 accumulator of `workspace` (rows [q_begin, q_end) of each item),
+ *            which sap_attn_bwd_begin zeroes (and fills D for) and sap_attn_bwd_end converts.
+ * Other arguments, errors and asynchrony as sap_attn_bwd_chunks. */
+/* sap_attn_fwd_items: the forward `computing` instruction: as sap_attn_fwd_partial, but only the 128-row Q tiles that
+ * intersect the items' row ranges are computed and written (rows of a touched tile without a visible key among the items
+ * get out = 0, lse = -inf); rows of other tiles are left alone.  With tensors addressed through shard-sized buffers
+ * (base pointer moved back by the shard's first row) a rank therefore needs memory for one shard of q / out and one of
+ * k / v, not for the sequence. */
+int sap_attn_fwd_items(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev,
+                       sap_plan_t* plan, int64_t n_tokens, int32_t item_begin, int32_t item_end,
+                       float* out_f32, float* lse,
+                       int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale, void* cuda_stream);
+int sap_attn_bwd_items(const void* dout, const void* q, const void* k, const void* v, const float* lse,
+                       const int32_t* cu_seqlens_dev, sap_plan_t* plan, int64_t n_tokens, int32_t item_begin, int32_t item_end,
+                       void* dk, void* dv, int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
+                       void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* dst = (accumulate ? dst : 0) + alpha * src, elementwise over n_elems values; dst, src: device, fp32 or bf16 each
+ * (*_is_bf16), 16-byte aligned, n_elems % 8 == 0.  The COPY instruction for received gradient contributions
+ * ("copy-dq / copy-dkv src_buf dst_buf", Table 1: a received dq / dkv is added into the owner's
+ * gradient) and the conversion of an fp32 gradient total to bf16.  Asynchronous on cuda_stream. */
+int sap_axpy(void* dst, int dst_is_bf16, const void* src, int src_is_bf16, int64_t n_elems, float alpha, int accumulate,
+             void* cuda_stream);
 
 /* ---- diagnostics ---------------------------------------------------------------------------- */
 const char* sap_strerror(int status);

@@ -37,21 +37,26 @@ SIGNATURES = {
     "sap_plan_codegen_bwd": (ctypes.c_int32, [vp, vp, ctypes.c_int32, vp, ctypes.c_int32]),
     "sap_plan_upload": (ctypes.c_int, [vp]),
     "sap_workspace_bytes": (ctypes.c_size_t, [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
-    "sap_attn_fwd": (ctypes.c_int, [vp, vp, vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+    "sap_attn_fwd": (ctypes.c_int, [vp, vp, vp, vp, vp, ctypes.c_int64, vp, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                     ctypes.c_float, vp, ctypes.c_size_t, vp]),
-    "sap_attn_fwd_partial": (ctypes.c_int, [vp, vp, vp, vp, vp, ctypes.c_int32, ctypes.c_int32, vp, vp,
+    "sap_attn_fwd_partial": (ctypes.c_int, [vp, vp, vp, vp, vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, vp, vp,
                                             ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_float, vp]),
+    "sap_attn_fwd_items": (ctypes.c_int, [vp, vp, vp, vp, vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, vp, vp,
+                                          ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_float, vp]),
     "sap_lse_merge": (ctypes.c_int, [vp, vp, vp, vp, vp, ctypes.c_int, vp, ctypes.c_int64, ctypes.c_int,
                                      ctypes.c_int, ctypes.c_int64, ctypes.c_int64, vp]),
-    "sap_attn_bwd": (ctypes.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int,
+    "sap_attn_bwd": (ctypes.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, ctypes.c_int64, vp, vp, vp, ctypes.c_int, ctypes.c_int,
                                     ctypes.c_int, ctypes.c_float, vp, ctypes.c_size_t, vp]),
-    "sap_attn_fwd_chunks": (ctypes.c_int, [vp, vp, vp, vp, vp, ctypes.c_int32, ctypes.c_int32, vp, vp, ctypes.c_int,
+    "sap_attn_fwd_chunks": (ctypes.c_int, [vp, vp, vp, vp, vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, vp, vp, ctypes.c_int,
                                            ctypes.c_int, ctypes.c_int, ctypes.c_float, vp]),
-    "sap_attn_bwd_begin": (ctypes.c_int, [vp, vp, vp, ctypes.c_int32, ctypes.c_int32, ctypes.c_int, ctypes.c_int,
+    "sap_attn_bwd_begin": (ctypes.c_int, [vp, vp, vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.c_int, ctypes.c_int,
                                           ctypes.c_int, vp, ctypes.c_size_t, vp]),
-    "sap_attn_bwd_chunks": (ctypes.c_int, [vp, vp, vp, vp, vp, vp, vp, ctypes.c_int32, ctypes.c_int32, vp, vp,
+    "sap_attn_bwd_chunks": (ctypes.c_int, [vp, vp, vp, vp, vp, vp, vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, vp, vp,
                                            ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_float, vp, ctypes.c_size_t, vp]),
-    "sap_attn_bwd_end": (ctypes.c_int, [vp, ctypes.c_int32, ctypes.c_int32, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+    "sap_attn_bwd_items": (ctypes.c_int, [vp, vp, vp, vp, vp, vp, vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, vp, vp,
+                                          ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_float, vp, ctypes.c_size_t, vp]),
+    "sap_axpy": (ctypes.c_int, [vp, ctypes.c_int, vp, ctypes.c_int, ctypes.c_int64, ctypes.c_float, ctypes.c_int, vp]),
+    "sap_attn_bwd_end": (ctypes.c_int, [vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                         ctypes.c_float, vp, ctypes.c_size_t, vp]),
     "sap_strerror": (ctypes.c_char_p, [ctypes.c_int]),
     "sap_last_cuda_error": (ctypes.c_int, []),

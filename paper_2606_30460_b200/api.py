@@ -154,6 +154,8 @@ def _dims(q, k):
 def _require_cuda_bf16(*ts):
     import torch
     for t in ts:
+        if type(t).__name__ == "ShardView":   # a shard addressed with global token rows (executor.ShardView)
+            t = t._t
         if not (t.is_cuda and t.dtype == torch.bfloat16 and t.is_contiguous()):
             raise ValueError("expected contiguous CUDA bf16 tensors")
 
@@ -169,7 +171,7 @@ def sap_attn_fwd(q, k, v, cu_seqlens_dev, plan: Plan, out=None, lse=None, softma
     if lse is None:
         lse = torch.empty((Hq, N), dtype=torch.float32, device=q.device)
     scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
-    _check(_lib.lib().sap_attn_fwd(_ptr(q), _ptr(k), _ptr(v), _ptr(cu_seqlens_dev), plan.handle, _ptr(out),
+    _check(_lib.lib().sap_attn_fwd(_ptr(q), _ptr(k), _ptr(v), _ptr(cu_seqlens_dev), plan.handle, N, _ptr(out),
                                    _ptr(lse), Hq, Hkv, d, scale, None, 0, _stream(stream)), "sap_attn_fwd")
     return out, lse
 
@@ -183,10 +185,21 @@ def sap_attn_fwd_partial(q, k, v, cu_seqlens_dev, plan: Plan, item_begin: int, i
     out = torch.empty((N, Hq, d), dtype=torch.float32, device=q.device)
     lse = torch.empty((Hq, N), dtype=torch.float32, device=q.device)
     scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
-    _check(_lib.lib().sap_attn_fwd_partial(_ptr(q), _ptr(k), _ptr(v), _ptr(cu_seqlens_dev), plan.handle,
+    _check(_lib.lib().sap_attn_fwd_partial(_ptr(q), _ptr(k), _ptr(v), _ptr(cu_seqlens_dev), plan.handle, N,
                                            int(item_begin), int(item_end), _ptr(out), _ptr(lse), Hq, Hkv, d, scale,
                                            _stream(stream)), "sap_attn_fwd_partial")
     return out, lse
+
+
+def sap_attn_fwd_items(q, k, v, cu_seqlens_dev, plan: Plan, item_begin: int, item_end: int, out_f32, lse,
+                       n_q_heads: int, n_kv_heads: int, head_dim: int, softmax_scale: Optional[float] = None, stream=None):
+    """The forward `computing` instruction: partial forward of plan items [item_begin, item_end) into caller-provided
+    buffers, touching only the Q tiles of those items.  Tensor arguments only need data_ptr() (the kernels index them
+    with global token rows: see executor.ShardView)."""
+    scale = float(head_dim) ** -0.5 if softmax_scale is None else float(softmax_scale)
+    _check(_lib.lib().sap_attn_fwd_items(_ptr(q), _ptr(k), _ptr(v), _ptr(cu_seqlens_dev), plan.handle, plan.n_tokens,
+                                         int(item_begin), int(item_end), _ptr(out_f32), _ptr(lse), int(n_q_heads),
+                                         int(n_kv_heads), int(head_dim), scale, _stream(stream)), "sap_attn_fwd_items")
 
 
 def sap_lse_merge(o_a, lse_a, o_b, lse_b, out_bf16: bool = False, row_begin: int = 0,
@@ -218,7 +231,7 @@ def sap_attn_bwd(dout, q, k, v, out, lse, cu_seqlens_dev, plan: Plan, softmax_sc
         workspace = torch.empty(need, dtype=torch.uint8, device=q.device)
     scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
     _check(_lib.lib().sap_attn_bwd(_ptr(dout), _ptr(q), _ptr(k), _ptr(v), _ptr(out), _ptr(lse),
-                                   _ptr(cu_seqlens_dev), plan.handle, _ptr(dq), _ptr(dk), _ptr(dv), Hq, Hkv, d,
+                                   _ptr(cu_seqlens_dev), plan.handle, N, _ptr(dq), _ptr(dk), _ptr(dv), Hq, Hkv, d,
                                    scale, _ptr(workspace), workspace.numel(), _stream(stream)), "sap_attn_bwd")
     return dq, dk, dv
 
@@ -249,7 +262,7 @@ def sap_attn_fwd_chunks(q, k, v, cu_seqlens_dev, plan: Plan, q_chunk_begin: int,
     _require_cuda_bf16(q, k, v, out)
     N, Hq, Hkv, d = _dims(q, k)
     scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
-    _check(_lib.lib().sap_attn_fwd_chunks(_ptr(q), _ptr(k), _ptr(v), _ptr(cu_seqlens_dev), plan.handle,
+    _check(_lib.lib().sap_attn_fwd_chunks(_ptr(q), _ptr(k), _ptr(v), _ptr(cu_seqlens_dev), plan.handle, N,
                                           int(q_chunk_begin), int(q_chunk_end), _ptr(out), _ptr(lse), Hq, Hkv, d, scale,
                                           _stream(stream)), "sap_attn_fwd_chunks")
     return out, lse
@@ -257,7 +270,7 @@ def sap_attn_fwd_chunks(q, k, v, cu_seqlens_dev, plan: Plan, q_chunk_begin: int,
 
 def sap_attn_bwd_begin(dout, out, plan: Plan, q_chunk_begin: int, q_chunk_end: int, n_kv_heads: int, workspace, stream=None):
     N, Hq, d = dout.shape
-    _check(_lib.lib().sap_attn_bwd_begin(_ptr(dout), _ptr(out), plan.handle, int(q_chunk_begin), int(q_chunk_end),
+    _check(_lib.lib().sap_attn_bwd_begin(_ptr(dout), _ptr(out), plan.handle, int(N), int(q_chunk_begin), int(q_chunk_end),
                                          int(Hq), int(n_kv_heads), int(d), _ptr(workspace), workspace.numel(),
                                          _stream(stream)), "sap_attn_bwd_begin")
 
@@ -268,7 +281,7 @@ def sap_attn_bwd_chunks(dout, q, k, v, lse, cu_seqlens_dev, plan: Plan, kv_chunk
     N, Hq, Hkv, d = _dims(q, k)
     scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
     _check(_lib.lib().sap_attn_bwd_chunks(_ptr(dout), _ptr(q), _ptr(k), _ptr(v), _ptr(lse), _ptr(cu_seqlens_dev),
-                                          plan.handle, int(kv_chunk_begin), int(kv_chunk_end), _ptr(dk), _ptr(dv), Hq, Hkv,
+                                          plan.handle, N, int(kv_chunk_begin), int(kv_chunk_end), _ptr(dk), _ptr(dv), Hq, Hkv,
                                           d, scale, _ptr(workspace), workspace.numel(), _stream(stream)),
            "sap_attn_bwd_chunks")
 
@@ -277,6 +290,33 @@ def sap_attn_bwd_end(plan: Plan, q_chunk_begin: int, q_chunk_end: int, dq, n_kv_
                      softmax_scale: Optional[float] = None, stream=None):
     N, Hq, d = dq.shape
     scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
-    _check(_lib.lib().sap_attn_bwd_end(plan.handle, int(q_chunk_begin), int(q_chunk_end), _ptr(dq), int(Hq),
+    _check(_lib.lib().sap_attn_bwd_end(plan.handle, int(N), int(q_chunk_begin), int(q_chunk_end), _ptr(dq), int(Hq),
                                        int(n_kv_heads), int(d), scale, _ptr(workspace), workspace.numel(),
                                        _stream(stream)), "sap_attn_bwd_end")
+
+
+# ---- per-item launches: the backward `computing` instruction and the gradient COPY ----------------
+def sap_attn_bwd_items(dout, q, k, v, lse, cu_seqlens_dev, plan: Plan, item_begin: int, item_end: int, dk, dv, workspace,
+                       softmax_scale: Optional[float] = None, stream=None):
+    """Fused backward of plan items [item_begin, item_end): dk / dv rows of the touched K/V tiles are written with the
+    items' contribution, dQ contributions are added into the accumulator of `workspace`."""
+    _require_cuda_bf16(dout, q, k, v, dk, dv)
+    N, Hq, Hkv, d = _dims(q, k)
+    scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
+    _check(_lib.lib().sap_attn_bwd_items(_ptr(dout), _ptr(q), _ptr(k), _ptr(v), _ptr(lse), _ptr(cu_seqlens_dev),
+                                         plan.handle, N, int(item_begin), int(item_end), _ptr(dk), _ptr(dv), Hq, Hkv,
+                                         d, scale, _ptr(workspace), workspace.numel(), _stream(stream)),
+           "sap_attn_bwd_items")
+
+
+def sap_axpy(dst, src, alpha: float = 1.0, accumulate: bool = True, stream=None):
+    """dst = (dst if accumulate else 0) + alpha * src on the GPU; dst, src contiguous fp32 or bf16 CUDA tensors."""
+    import torch
+    if not (dst.is_cuda and src.is_cuda and dst.is_contiguous() and src.is_contiguous() and dst.numel() == src.numel()):
+        raise ValueError("expected contiguous CUDA tensors of equal size")
+    for t in (dst, src):
+        if t.dtype not in (torch.float32, torch.bfloat16):
+            raise ValueError("fp32 or bf16 only")
+    _check(_lib.lib().sap_axpy(_ptr(dst), int(dst.dtype == torch.bfloat16), _ptr(src), int(src.dtype == torch.bfloat16),
+                               dst.numel(), float(alpha), int(accumulate), _stream(stream)), "sap_axpy")
+    return dst

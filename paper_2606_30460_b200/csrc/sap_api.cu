@@ -1,7 +1,9 @@
-// C-ABI entry points that touch the GPU (include/sap.h): plan upload, forward, partial forward,
-// LSE merge, backward.  Argument checking + tensor-map encoding + launches only.
+// C-ABI entry points that touch the GPU (include/sap.h): plan upload, forward, partial forward, LSE merge, backward,
+// per-rank and per-item launches.  Argument checking + tensor-map encoding + launches only.
 #include <cstdio>
 #include <cstring>
+#include <list>
+#include <set>
 #include "sap_host.h"
 #include "sap_fwd.cuh"
 #include "sap_fwd_pair.cuh"
@@ -15,20 +17,21 @@ namespace sap {
 // sap_debug_set_bwd_stages bits: 1 D pre-pass | 2 split dK/dV kernel | 4 split dQ kernel | 8 fused main kernel
 // (+ zeroing of its fp32 dQ accumulator) | 16 dQ post pass.  Default: pre + fused + post.
 constexpr int kBwdDefaultStages = 1 | 8 | 16;
+constexpr size_t kMaxRangePrograms = 64;   // cached range-restricted programs per plan and kind (least recently used goes)
 static inline size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
 
 thread_local int g_last_cuda_error = 0;
 std::atomic<int64_t> g_launch_count{0};
 std::atomic<int> g_bwd_stages{kBwdDefaultStages};
-std::atomic<int> g_fwd_form{0};
-std::atomic<int> g_bwd_form{0};  // 0: CTA-pair fused kernel for head_dim 128, 1: always the one-CTA fused kernel (diagnostic)  // 0: pair kernel when Hq/Hkv is even, 1: always the one-head kernel (diagnostic)
+std::atomic<int> g_fwd_form{0};  // 0: pair kernel when Hq/Hkv is even, 1: always the one-head kernel (diagnostic)
+std::atomic<int> g_bwd_form{0};  // 0: CTA-pair fused kernel for head_dim 128, 1: always the one-CTA fused kernel (diagnostic)
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 static EncodeTiledFn get_encode_fn() {
-  static EncodeTiledFn fn = []() -> EncodeTiledFn {
+  static EncodeTiledFn fn = []() -> EncodeTiledFn {   // function-local static: initialised once, thread-safe
     void* p = nullptr;
     cudaDriverEntryPointQueryResult q;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess) return nullptr;
@@ -51,26 +54,38 @@ int make_tile_map(CUtensorMap* map, const void* base, int64_t n_rows, int64_t ro
   return SAP_OK;
 }
 
-int check_device_is_sm100() {
-  int dev = 0;
-  SAP_CUDA_CHECK(cudaGetDevice(&dev));
-  static int cached_dev = -1, cached_major = 0;
-  if (cached_dev != dev) {
-    int major = 0;
-    SAP_CUDA_CHECK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
-    cached_major = major; cached_dev = dev;
-  }
-  return cached_major == 10 ? SAP_OK : SAP_ERR_WRONG_ARCH;
+// Per-device one-time setup: architecture check and the opt-in shared-memory sizes of every kernel
+// (cudaFuncSetAttribute is per device).  Guarded by a mutex; `*dev_out` = the current device.
+template <int D>
+static cudaError_t set_kernel_attributes() {
+  cudaError_t e;
+  const cudaFuncAttribute a = cudaFuncAttributeMaxDynamicSharedMemorySize;
+  if ((e = cudaFuncSetAttribute(sap_fwd_kernel<D, false>, a, FwdSmem<D>::kTotal)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(sap_fwd_kernel<D, true>, a, FwdSmem<D>::kTotal)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(sap_fwd_pair_kernel<D, false>, a, FwdPairSmem<D>::kTotal)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(sap_fwd_pair_kernel<D, true>, a, FwdPairSmem<D>::kTotal)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(sap_bwd_dq_kernel<D>, a, DqSmem<D>::kTotal)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(sap_bwd_dkv_kernel<D>, a, DkvSmem<D>::kTotal)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(sap_bwd_fused_kernel<D>, a, FusedSmem<D>::kTotal)) != cudaSuccess) return e;
+  return cudaSuccess;
 }
 
-int upload_program(const TileProgram& host, DevProgram& dev) {
-  dev.n_tiles = static_cast<int32_t>(host.tiles.size());
-  const size_t tb = host.tiles.size() * sizeof(TileDesc), sb = (host.segs.size() + 1) * sizeof(SegDesc);
-  SAP_CUDA_CHECK(cudaMalloc(&dev.tiles, tb ? tb : sizeof(TileDesc)));
-  SAP_CUDA_CHECK(cudaMalloc(&dev.segs, sb));
-  if (tb) SAP_CUDA_CHECK(cudaMemcpy(dev.tiles, host.tiles.data(), tb, cudaMemcpyHostToDevice));
-  if (!host.segs.empty())
-    SAP_CUDA_CHECK(cudaMemcpy(dev.segs, host.segs.data(), host.segs.size() * sizeof(SegDesc), cudaMemcpyHostToDevice));
+int ensure_device(int* dev_out) {
+  static std::mutex mu;
+  static std::set<int> ready, wrong_arch;
+  int dev = 0;
+  SAP_CUDA_CHECK(cudaGetDevice(&dev));
+  if (dev_out) *dev_out = dev;
+  std::lock_guard<std::mutex> lock(mu);
+  if (ready.count(dev)) return SAP_OK;
+  if (wrong_arch.count(dev)) return SAP_ERR_WRONG_ARCH;
+  int major = 0;
+  SAP_CUDA_CHECK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+  if (major != 10) { wrong_arch.insert(dev); return SAP_ERR_WRONG_ARCH; }
+  SAP_CUDA_CHECK(set_kernel_attributes<64>());
+  SAP_CUDA_CHECK(set_kernel_attributes<128>());
+  SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PairSmem::kTotal));
+  ready.insert(dev);
   return SAP_OK;
 }
 
@@ -80,12 +95,56 @@ void free_program(DevProgram& dev) {
   dev = DevProgram();
 }
 
+// Synchronous upload (sap_plan_upload).  Frees what it allocated when a later step fails.
+int upload_program(const TileProgram& host, DevProgram& dev) {
+  dev = DevProgram();
+  dev.n_tiles = static_cast<int32_t>(host.tiles.size());
+  const size_t tb = host.tiles.size() * sizeof(TileDesc), sb = (host.segs.size() + 1) * sizeof(SegDesc);
+  cudaError_t e = cudaMalloc(&dev.tiles, tb ? tb : sizeof(TileDesc));
+  if (e == cudaSuccess) e = cudaMalloc(&dev.segs, sb);
+  if (e == cudaSuccess && tb) e = cudaMemcpy(dev.tiles, host.tiles.data(), tb, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess && !host.segs.empty())
+    e = cudaMemcpy(dev.segs, host.segs.data(), host.segs.size() * sizeof(SegDesc), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { free_program(dev); SAP_CUDA_CHECK(e); }
+  return SAP_OK;
+}
+
+// Stream-ordered upload of a range-restricted program: no device synchronisation.  `host` must stay alive until the
+// copies have run (it lives in the cache entry); `ready` is recorded behind the copies for uses on other streams.
+static int upload_program_async(const TileProgram& host, DevProgram& dev, cudaEvent_t* ready, cudaStream_t stream) {
+  dev = DevProgram();
+  dev.n_tiles = static_cast<int32_t>(host.tiles.size());
+  const size_t tb = host.tiles.size() * sizeof(TileDesc), sb = (host.segs.size() + 1) * sizeof(SegDesc);
+  cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&dev.tiles), tb ? tb : sizeof(TileDesc), stream);
+  if (e == cudaSuccess) e = cudaMallocAsync(reinterpret_cast<void**>(&dev.segs), sb, stream);
+  if (e == cudaSuccess && tb) e = cudaMemcpyAsync(dev.tiles, host.tiles.data(), tb, cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess && !host.segs.empty())
+    e = cudaMemcpyAsync(dev.segs, host.segs.data(), host.segs.size() * sizeof(SegDesc), cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(ready, cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventRecord(*ready, stream);
+  if (e != cudaSuccess) {
+    if (dev.tiles) cudaFreeAsync(dev.tiles, stream);
+    if (dev.segs) cudaFreeAsync(dev.segs, stream);
+    dev = DevProgram();
+    SAP_CUDA_CHECK(e);
+  }
+  return SAP_OK;
+}
+
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-static int check_dims(const sap_plan_t* plan, int Hq, int Hkv, int d, float scale) {
+// Common checks of the attention calls: dims, the caller's length against the plan's (a plan built for another length
+// would make the kernels read out of bounds), device setup, and that the plan's device mirror lives on this device.
+static int check_call(sap_plan_t* plan, int64_t n_tokens, int Hq, int Hkv, int d, float scale, bool need_upload = true) {
   if (!plan) return SAP_ERR_INVALID_ARG;
   if (Hq < 1 || Hkv < 1 || !(scale > 0.f)) return SAP_ERR_INVALID_ARG;
   if ((d != 64 && d != 128) || Hq % Hkv != 0) return SAP_ERR_UNSUPPORTED;
+  if (n_tokens != plan->n_tokens) return SAP_ERR_PLAN_MISMATCH;
+  int dev = 0, rc;
+  if ((rc = ensure_device(&dev)) != SAP_OK) return rc;
+  if (need_upload && (rc = sap_plan_upload(plan)) != SAP_OK) return rc;
+  const PlanDevice* pd = static_cast<const PlanDevice*>(plan->dev_state);
+  if (pd && pd->uploaded && pd->device != dev) return SAP_ERR_PLAN_MISMATCH;
   return SAP_OK;
 }
 
@@ -93,39 +152,32 @@ template <int D, bool PARTIAL>
 static int launch_fwd(const DevProgram& prog, const void* q, const void* k, const void* v, const int32_t* cu,
                       const sap_plan_t* plan, void* out, float* out_f32, float* lse, int Hq, int Hkv, float scale,
                       cudaStream_t stream) {
+  if (prog.n_tiles == 0) return SAP_OK;
   CUtensorMap mq, mk, mv;
   int rc;
   if ((rc = make_tile_map(&mq, q, plan->n_tokens, (int64_t)Hq * D)) != SAP_OK) return rc;
   if ((rc = make_tile_map(&mk, k, plan->n_tokens, (int64_t)Hkv * D)) != SAP_OK) return rc;
   if ((rc = make_tile_map(&mv, v, plan->n_tokens, (int64_t)Hkv * D)) != SAP_OK) return rc;
-  auto kern = sap_fwd_kernel<D, PARTIAL>;
-  auto kern_pair = sap_fwd_pair_kernel<D, PARTIAL>;
-  static bool attr_set = false;
-  if (!attr_set) {
-    SAP_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdSmem<D>::kTotal));
-    SAP_CUDA_CHECK(cudaFuncSetAttribute(kern_pair, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdPairSmem<D>::kTotal));
-    attr_set = true;
-  }
   if ((Hq / Hkv) % 2 == 0 && g_fwd_form.load() == 0) {  // two q-heads of a GQA group per CTA share the K/V stream
     const unsigned grid = static_cast<unsigned>(prog.n_tiles) * (Hq / 2);
-    kern_pair<<<grid, kFwdPairThreads, FwdPairSmem<D>::kTotal, stream>>>(mq, mk, mv, prog.tiles, prog.segs, cu, plan->n_docs,
-                                                                      static_cast<__nv_bfloat16*>(out), out_f32, lse,
-                                                                      plan->n_tokens, Hq, Hkv, scale * kLog2e);
-    g_launch_count.fetch_add(1);
-    SAP_CUDA_CHECK(cudaGetLastError());
-    return SAP_OK;
+    sap_fwd_pair_kernel<D, PARTIAL><<<grid, kFwdPairThreads, FwdPairSmem<D>::kTotal, stream>>>(
+        mq, mk, mv, prog.tiles, prog.segs, cu, plan->n_docs, static_cast<__nv_bfloat16*>(out), out_f32, lse,
+        plan->n_tokens, Hq, Hkv, scale * kLog2e);
+  } else {
+    const unsigned grid = static_cast<unsigned>(prog.n_tiles) * Hq;
+    sap_fwd_kernel<D, PARTIAL><<<grid, kFwdThreads, FwdSmem<D>::kTotal, stream>>>(
+        mq, mk, mv, prog.tiles, prog.segs, cu, plan->n_docs, static_cast<__nv_bfloat16*>(out), out_f32, lse,
+        plan->n_tokens, Hq, Hkv, scale * kLog2e);
   }
-  const unsigned grid = static_cast<unsigned>(prog.n_tiles) * Hq;
-  kern<<<grid, kFwdThreads, FwdSmem<D>::kTotal, stream>>>(mq, mk, mv, prog.tiles, prog.segs, cu, plan->n_docs,
-                                                          static_cast<__nv_bfloat16*>(out), out_f32, lse,
-                                                          plan->n_tokens, Hq, Hkv, scale * kLog2e);
   g_launch_count.fetch_add(1);
   SAP_CUDA_CHECK(cudaGetLastError());
   return SAP_OK;
 }
 
-// a6: the fused main kernel over a KV-stationary program.  head_dim 128 runs on CTA pairs over the 256-key program
-// `prog2`, head_dim 64 (and the diagnostic form) on single CTAs over the 128-key program `prog1`.
+// a6: the fused main kernel over a KV-stationary program.  head_dim 128 runs on CTA pairs over a 256-key program
+// `prog2`, head_dim 64 (and the diagnostic form) on single CTAs over a 128-key program `prog1`.
+static inline bool use_pair_kernel(int d) { return d == 128 && g_bwd_form.load() == 0; }
+
 template <int D>
 static int launch_bwd_main(const DevProgram& prog1, const DevProgram& prog2, const void* dout, const void* q, const void* k,
                            const void* v, const float* lse, const int32_t* cu, const sap_plan_t* plan, void* dk, void* dv,
@@ -137,13 +189,7 @@ static int launch_bwd_main(const DevProgram& prog1, const DevProgram& prog2, con
   if ((rc = make_tile_map(&mdo64, dout, N, (int64_t)Hq * D, kBwdN)) != SAP_OK) return rc;
   if ((rc = make_tile_map(&mk128, k, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
   if ((rc = make_tile_map(&mv128, v, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
-  static bool attr_set = false;
-  if (!attr_set) {
-    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_fused_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, FusedSmem<D>::kTotal));
-    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PairSmem::kTotal));
-    attr_set = true;
-  }
-  if (D == 128 && g_bwd_form.load() == 0) {
+  if (use_pair_kernel(D)) {
     if (prog2.n_tiles == 0) return SAP_OK;
     CUtensorMap mq32, mdo32;
     if ((rc = make_tile_map(&mq32, q, N, (int64_t)Hq * D, 32)) != SAP_OK) return rc;
@@ -162,85 +208,23 @@ static int launch_bwd_main(const DevProgram& prog1, const DevProgram& prog2, con
   return SAP_OK;
 }
 
+// a5 for tokens [t0, t0 + nt): D = rowsum(dO * O); optionally zero the dQ accumulator rows
 template <int D>
-static int launch_bwd(const PlanDevice* pd, const void* dout, const void* q, const void* k, const void* v,
-                      const void* out, const float* lse, const int32_t* cu, const sap_plan_t* plan, void* dq, void* dk,
-                      void* dv, int Hq, int Hkv, float scale, float* dsum, float* dq_acc, cudaStream_t stream) {
-  const int64_t N = plan->n_tokens;
-  int rc;
-  const int stages = g_bwd_stages.load();
-  // a5: D = rowsum(dO * O)
-  if (stages & 1) {
-    const int64_t rows = N * Hq;
-    const int64_t want = (rows * (D / 8) + kPreThreads - 1) / kPreThreads;
-    const unsigned grid = static_cast<unsigned>(want < 148 * 16 ? want : 148 * 16);
-    sap_bwd_pre_kernel<D><<<grid, kPreThreads, 0, stream>>>(static_cast<const __nv_bfloat16*>(dout),
-                                                            static_cast<const __nv_bfloat16*>(out), dsum, N, Hq, 0, N);
-    g_launch_count.fetch_add(1);
-    SAP_CUDA_CHECK(cudaGetLastError());
-  }
-  CUtensorMap mq128, mdo128, mk64, mv64, mq64, mdo64, mk128, mv128;
-  if ((rc = make_tile_map(&mq128, q, N, (int64_t)Hq * D, kTile)) != SAP_OK) return rc;
-  if ((rc = make_tile_map(&mdo128, dout, N, (int64_t)Hq * D, kTile)) != SAP_OK) return rc;
-  if ((rc = make_tile_map(&mk64, k, N, (int64_t)Hkv * D, kBwdN)) != SAP_OK) return rc;
-  if ((rc = make_tile_map(&mv64, v, N, (int64_t)Hkv * D, kBwdN)) != SAP_OK) return rc;
-  if ((rc = make_tile_map(&mq64, q, N, (int64_t)Hq * D, kBwdN)) != SAP_OK) return rc;
-  if ((rc = make_tile_map(&mdo64, dout, N, (int64_t)Hq * D, kBwdN)) != SAP_OK) return rc;
-  if ((rc = make_tile_map(&mk128, k, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
-  if ((rc = make_tile_map(&mv128, v, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
-  static bool attr_set = false;
-  if (!attr_set) {
-    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_dq_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, DqSmem<D>::kTotal));
-    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_dkv_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, DkvSmem<D>::kTotal));
-    attr_set = true;
-  }
-  // a6 fused: dK, dV and the fp32 dQ accumulator in one pass (5 GEMMs per tile pair)
-  if (stages & 8) {
-    SAP_CUDA_CHECK(cudaMemsetAsync(dq_acc, 0, static_cast<size_t>(N) * Hq * D * sizeof(float), stream));
-    if ((rc = launch_bwd_main<D>(pd->kv, pd->kv2, dout, q, k, v, lse, cu, plan, dk, dv, Hq, Hkv, scale, dsum, dq_acc, stream)) != SAP_OK) return rc;
-  }
-  // a7: dq = bf16(scale * dq_acc)
-  if (stages & 16) {
-    const int64_t n8 = N * Hq * D / 8;
-    const int64_t want = (n8 + kPostThreads - 1) / kPostThreads;
-    const unsigned grid = static_cast<unsigned>(want < 148 * 16 ? want : 148 * 16);
-    sap_bwd_post_kernel<<<grid, kPostThreads, 0, stream>>>(dq_acc, static_cast<__nv_bfloat16*>(dq), n8, scale);
-    g_launch_count.fetch_add(1);
-    SAP_CUDA_CHECK(cudaGetLastError());
-  }
-  // a6 (dK/dV half first: it is the longer kernel)
-  if (stages & 2) {
-  sap_bwd_dkv_kernel<D><<<static_cast<unsigned>(pd->kv.n_tiles) * Hkv, kDkvThreads, DkvSmem<D>::kTotal, stream>>>(
-      mq64, mdo64, mk128, mv128, pd->kv.tiles, pd->kv.segs, cu, plan->n_docs, lse, dsum,
-      static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
-  g_launch_count.fetch_add(1);
-  SAP_CUDA_CHECK(cudaGetLastError());
-  }
-  if (stages & 4) {
-  sap_bwd_dq_kernel<D><<<static_cast<unsigned>(pd->fwd.n_tiles) * Hq, kDqThreads, DqSmem<D>::kTotal, stream>>>(
-      mq128, mdo128, mk64, mv64, pd->fwd.tiles, pd->fwd.segs, cu, plan->n_docs, lse, dsum,
-      static_cast<__nv_bfloat16*>(dq), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
-  g_launch_count.fetch_add(1);
-  SAP_CUDA_CHECK(cudaGetLastError());
-  }
-  return SAP_OK;
-}
-
-// ---- pieces of the backward for chunk-restricted launches (sap_attn_bwd_begin / _chunks / _end) ----------------
-template <int D>
-static int launch_bwd_begin(const void* dout, const void* out, int64_t N, int Hq, int64_t t0, int64_t nt, float* dsum,
-                            float* dq_acc, cudaStream_t stream) {
+static int launch_bwd_pre(const void* dout, const void* out, int64_t N, int Hq, int64_t t0, int64_t nt, float* dsum,
+                          float* dq_acc, bool zero_acc, cudaStream_t stream) {
+  if (nt == 0) return SAP_OK;
   const int64_t want = (nt * Hq * (D / 8) + kPreThreads - 1) / kPreThreads;
   const unsigned grid = static_cast<unsigned>(want < 148 * 16 ? want : 148 * 16);
   sap_bwd_pre_kernel<D><<<grid, kPreThreads, 0, stream>>>(static_cast<const __nv_bfloat16*>(dout),
                                                           static_cast<const __nv_bfloat16*>(out), dsum, N, Hq, t0, nt);
   g_launch_count.fetch_add(1);
   SAP_CUDA_CHECK(cudaGetLastError());
-  SAP_CUDA_CHECK(cudaMemsetAsync(dq_acc + t0 * Hq * D, 0, static_cast<size_t>(nt) * Hq * D * sizeof(float), stream));
+  if (zero_acc) SAP_CUDA_CHECK(cudaMemsetAsync(dq_acc + t0 * Hq * D, 0, static_cast<size_t>(nt) * Hq * D * sizeof(float), stream));
   return SAP_OK;
 }
 
-static int launch_bwd_end(const float* dq_acc, void* dq, int Hq, int d, int64_t t0, int64_t nt, float scale, cudaStream_t stream) {
+// a7 for tokens [t0, t0 + nt): dq = bf16(scale * dq_acc)
+static int launch_bwd_post(const float* dq_acc, void* dq, int Hq, int d, int64_t t0, int64_t nt, float scale, cudaStream_t stream) {
   const int64_t n8 = nt * Hq * d / 8;
   if (n8 == 0) return SAP_OK;
   const int64_t want = (n8 + kPostThreads - 1) / kPostThreads;
@@ -252,30 +236,139 @@ static int launch_bwd_end(const float* dq_acc, void* dq, int Hq, int d, int64_t 
   return SAP_OK;
 }
 
-// item-range (forward) or kv-chunk-range (backward) restricted programs, built once per range and kept with the plan
-// kind: 0 Q-stationary program of q-chunks, 1 KV-stationary of kv-chunks (128-key tiles), 2 the same with 256-key pair-tiles
-static int get_chunk_program(sap_plan_t* plan, int kind, int32_t c_begin, int32_t c_end, DevProgram* out) {
-  PlanDevice* pd = static_cast<PlanDevice*>(plan->dev_state);
-  std::lock_guard<std::mutex> lock(plan->mu);
-  const bool kv = kind != 0;
-  auto& cache = kind == 2 ? pd->kv2_chunks : (kind == 1 ? pd->kv_chunks : pd->q_chunks);
-  auto key = std::make_pair(c_begin, c_end);
-  auto itp = cache.find(key);
-  if (itp == cache.end()) {
-    TileProgram host;
-    if (kv) build_kv_program(*plan, host, c_begin, c_end, kind == 2 ? 2 * kTile : kTile);
-    else build_q_program(*plan, plan->chunk_offsets[c_begin], plan->chunk_offsets[c_end], host, /*drop_empty=*/true);
-    DevProgram dp;
-    int rc = upload_program(host, dp);
-    if (rc != SAP_OK) return rc;
-    itp = cache.emplace(key, dp).first;
+template <int D>
+static int launch_bwd(const PlanDevice* pd, const void* dout, const void* q, const void* k, const void* v,
+                      const void* out, const float* lse, const int32_t* cu, const sap_plan_t* plan, void* dq, void* dk,
+                      void* dv, int Hq, int Hkv, float scale, float* dsum, float* dq_acc, cudaStream_t stream) {
+  const int64_t N = plan->n_tokens;
+  int rc;
+  const int stages = g_bwd_stages.load();
+  if (stages & 1)
+    if ((rc = launch_bwd_pre<D>(dout, out, N, Hq, 0, N, dsum, dq_acc, false, stream)) != SAP_OK) return rc;
+  if (stages & 8) {  // a6 fused: dK, dV and the fp32 dQ accumulator in one pass (5 GEMMs per tile pair)
+    SAP_CUDA_CHECK(cudaMemsetAsync(dq_acc, 0, static_cast<size_t>(N) * Hq * D * sizeof(float), stream));
+    if ((rc = launch_bwd_main<D>(pd->kv, pd->kv2, dout, q, k, v, lse, cu, plan, dk, dv, Hq, Hkv, scale, dsum, dq_acc, stream)) != SAP_OK) return rc;
   }
-  *out = itp->second;
+  if (stages & 16)
+    if ((rc = launch_bwd_post(dq_acc, dq, Hq, D, 0, N, scale, stream)) != SAP_OK) return rc;
+  if (stages & 6) {  // the split, atomics-free form (diagnostic): 7 GEMMs per tile pair
+    CUtensorMap mq128, mdo128, mk64, mv64, mq64, mdo64, mk128, mv128;
+    if ((rc = make_tile_map(&mq128, q, N, (int64_t)Hq * D, kTile)) != SAP_OK) return rc;
+    if ((rc = make_tile_map(&mdo128, dout, N, (int64_t)Hq * D, kTile)) != SAP_OK) return rc;
+    if ((rc = make_tile_map(&mk64, k, N, (int64_t)Hkv * D, kBwdN)) != SAP_OK) return rc;
+    if ((rc = make_tile_map(&mv64, v, N, (int64_t)Hkv * D, kBwdN)) != SAP_OK) return rc;
+    if ((rc = make_tile_map(&mq64, q, N, (int64_t)Hq * D, kBwdN)) != SAP_OK) return rc;
+    if ((rc = make_tile_map(&mdo64, dout, N, (int64_t)Hq * D, kBwdN)) != SAP_OK) return rc;
+    if ((rc = make_tile_map(&mk128, k, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
+    if ((rc = make_tile_map(&mv128, v, N, (int64_t)Hkv * D, kTile)) != SAP_OK) return rc;
+    if (stages & 2) {
+      sap_bwd_dkv_kernel<D><<<static_cast<unsigned>(pd->kv.n_tiles) * Hkv, kDkvThreads, DkvSmem<D>::kTotal, stream>>>(
+          mq64, mdo64, mk128, mv128, pd->kv.tiles, pd->kv.segs, cu, plan->n_docs, lse, dsum,
+          static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
+      g_launch_count.fetch_add(1);
+      SAP_CUDA_CHECK(cudaGetLastError());
+    }
+    if (stages & 4) {
+      sap_bwd_dq_kernel<D><<<static_cast<unsigned>(pd->fwd.n_tiles) * Hq, kDqThreads, DqSmem<D>::kTotal, stream>>>(
+          mq128, mdo128, mk64, mv64, pd->fwd.tiles, pd->fwd.segs, cu, plan->n_docs, lse, dsum,
+          static_cast<__nv_bfloat16*>(dq), plan->n_tokens, Hq, Hkv, scale, scale * kLog2e);
+      g_launch_count.fetch_add(1);
+      SAP_CUDA_CHECK(cudaGetLastError());
+    }
+  }
   return SAP_OK;
 }
 
-static inline bool chunk_range_ok(const sap_plan_t* plan, int32_t a, int32_t b) {
-  return a >= 0 && b >= a && b <= plan->n_chunks;
+// Range-restricted programs, built on first use of a range and kept with the plan (at most kMaxRangePrograms per
+// kind, least recently used evicted).  Uploads and evictions are ordered on the caller's stream: no synchronisation.
+static int get_range_program(sap_plan_t* plan, int kind, int32_t a, int32_t b, cudaStream_t stream, DevProgram* out) {
+  PlanDevice* pd = static_cast<PlanDevice*>(plan->dev_state);
+  std::lock_guard<std::mutex> lock(plan->mu);
+  auto& cache = pd->ranges[kind];
+  const auto key = std::make_pair(a, b);
+  RangeProgram* hit = nullptr;
+  for (auto it = cache.begin(); it != cache.end(); ++it)
+    if (it->key == key) { cache.splice(cache.begin(), cache, it); hit = &cache.front(); break; }
+  if (!hit) {
+    if (cache.size() >= kMaxRangePrograms) {
+      RangeProgram& old = cache.back();
+      if (old.dev.tiles) cudaFreeAsync(old.dev.tiles, stream);
+      if (old.dev.segs) cudaFreeAsync(old.dev.segs, stream);
+      if (old.ready) cudaEventDestroy(old.ready);
+      cache.pop_back();
+    }
+    cache.emplace_front();
+    RangeProgram& e = cache.front();
+    e.key = key;
+    const int32_t kv_rows = (kind == kRangeKvPair || kind == kRangeItemsKvPair) ? 2 * kTile : kTile;
+    switch (kind) {
+      case kRangeItemsQ: build_q_program(*plan, a, b, e.host); break;                                               // partial forward, every row
+      case kRangeItemsQDrop: build_q_program(*plan, a, b, e.host, true); break;                                     // ... touched Q tiles only
+      case kRangeQ: build_q_program(*plan, plan->chunk_offsets[a], plan->chunk_offsets[b], e.host, true); break;    // q-chunks
+      case kRangeKv: case kRangeKvPair: build_kv_program(*plan, e.host, a, b, kv_rows); break;                      // kv-chunks
+      default: build_kv_program(*plan, e.host, 0, -1, kv_rows, a, b, true); break;                                  // items, KV-stationary
+    }
+    e.stream = stream;
+    int rc = upload_program_async(e.host, e.dev, &e.ready, stream);
+    if (rc != SAP_OK) { cache.pop_front(); return rc; }
+    hit = &e;
+  }
+  if (hit->stream != stream) SAP_CUDA_CHECK(cudaStreamWaitEvent(stream, hit->ready, 0));
+  *out = hit->dev;
+  return SAP_OK;
+}
+
+static inline bool chunk_range_ok(const sap_plan_t* plan, int32_t a, int32_t b) { return a >= 0 && b >= a && b <= plan->n_chunks; }
+static inline bool item_range_ok(const sap_plan_t* plan, int32_t a, int32_t b) { return a >= 0 && b >= a && b <= (int32_t)plan->items.size(); }
+
+static int bwd_ws(const sap_plan_t* plan, int Hq, int Hkv, int d, void* workspace, size_t bytes, float** dsum, float** dq_acc) {
+  if (!aligned16(workspace)) return SAP_ERR_UNSUPPORTED;
+  if (!workspace || bytes < sap_workspace_bytes(plan, Hq, Hkv, d, SAP_PASS_BWD)) return SAP_ERR_WORKSPACE_TOO_SMALL;
+  *dsum = static_cast<float*>(workspace);
+  *dq_acc = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + align256(static_cast<size_t>(plan->n_tokens) * Hq * sizeof(float)));
+  return SAP_OK;
+}
+
+// dst (+)= alpha * src, elementwise, fp32 or bf16 on either side; 8 elements per thread and step
+template <bool DST_BF16, bool SRC_BF16>
+__global__ void __launch_bounds__(256)
+sap_axpy_kernel(void* dst, const void* src, int64_t n8, float alpha, int accumulate) {
+  const int64_t stride = static_cast<int64_t>(gridDim.x) * blockDim.x;
+  for (int64_t i = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x; i < n8; i += stride) {
+    float s[8], d[8];
+    if (SRC_BF16) {
+      const uint4 w = reinterpret_cast<const uint4*>(src)[i];
+      const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+      for (int e = 0; e < 4; ++e) { s[2 * e] = __uint_as_float(ww[e] << 16); s[2 * e + 1] = __uint_as_float(ww[e] & 0xffff0000u); }
+    } else {
+      const float4 a = reinterpret_cast<const float4*>(src)[2 * i], b = reinterpret_cast<const float4*>(src)[2 * i + 1];
+      s[0] = a.x; s[1] = a.y; s[2] = a.z; s[3] = a.w; s[4] = b.x; s[5] = b.y; s[6] = b.z; s[7] = b.w;
+    }
+#pragma unroll
+    for (int e = 0; e < 8; ++e) d[e] = 0.f;
+    if (accumulate) {
+      if (DST_BF16) {
+        const uint4 w = reinterpret_cast<const uint4*>(dst)[i];
+        const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { d[2 * e] = __uint_as_float(ww[e] << 16); d[2 * e + 1] = __uint_as_float(ww[e] & 0xffff0000u); }
+      } else {
+        const float4 a = reinterpret_cast<const float4*>(dst)[2 * i], b = reinterpret_cast<const float4*>(dst)[2 * i + 1];
+        d[0] = a.x; d[1] = a.y; d[2] = a.z; d[3] = a.w; d[4] = b.x; d[5] = b.y; d[6] = b.z; d[7] = b.w;
+      }
+    }
+#pragma unroll
+    for (int e = 0; e < 8; ++e) d[e] = fmaf(alpha, s[e], d[e]);
+    if (DST_BF16) {
+      uint4 w;
+      w.x = pack_bf16x2(d[0], d[1]); w.y = pack_bf16x2(d[2], d[3]); w.z = pack_bf16x2(d[4], d[5]); w.w = pack_bf16x2(d[6], d[7]);
+      reinterpret_cast<uint4*>(dst)[i] = w;
+    } else {
+      reinterpret_cast<float4*>(dst)[2 * i] = make_float4(d[0], d[1], d[2], d[3]);
+      reinterpret_cast<float4*>(dst)[2 * i + 1] = make_float4(d[4], d[5], d[6], d[7]);
+    }
+  }
 }
 
 }  // namespace sap
@@ -302,16 +395,20 @@ int sap_debug_set_bwd_stages(int mask) { return g_bwd_stages.exchange(mask < 0 ?
 
 int sap_plan_upload(sap_plan_t* plan) {
   if (!plan) return SAP_ERR_INVALID_ARG;
+  int dev = 0;
+  int rc = ensure_device(&dev);
+  if (rc != SAP_OK) return rc;
   std::lock_guard<std::mutex> lock(plan->mu);
   PlanDevice* pd = static_cast<PlanDevice*>(plan->dev_state);
-  if (pd && pd->uploaded) return SAP_OK;
-  int rc = check_device_is_sm100();
-  if (rc != SAP_OK) return rc;
+  if (pd && pd->uploaded) return pd->device == dev ? SAP_OK : SAP_ERR_PLAN_MISMATCH;   // a plan's mirror lives on one device
   if (!pd) { pd = new PlanDevice(); plan->dev_state = pd; }
-  SAP_CUDA_CHECK(cudaGetDevice(&pd->device));
-  if ((rc = upload_program(plan->fwd, pd->fwd)) != SAP_OK) return rc;
-  if ((rc = upload_program(plan->kv, pd->kv)) != SAP_OK) return rc;
-  if ((rc = upload_program(plan->kv2, pd->kv2)) != SAP_OK) return rc;
+  pd->device = dev;
+  if ((rc = upload_program(plan->fwd, pd->fwd)) == SAP_OK && (rc = upload_program(plan->kv, pd->kv)) == SAP_OK)
+    rc = upload_program(plan->kv2, pd->kv2);
+  if (rc != SAP_OK) {  // leave nothing half-uploaded behind: a retry starts from scratch
+    free_program(pd->fwd); free_program(pd->kv); free_program(pd->kv2);
+    return rc;
+  }
   pd->uploaded = true;
   return SAP_OK;
 }
@@ -320,13 +417,14 @@ void sap_plan_destroy(sap_plan_t* plan) {
   if (!plan) return;
   PlanDevice* pd = static_cast<PlanDevice*>(plan->dev_state);
   if (pd) {
+    int cur = -1;
+    const bool switched = pd->uploaded && cudaGetDevice(&cur) == cudaSuccess && cur != pd->device && cudaSetDevice(pd->device) == cudaSuccess;
     free_program(pd->fwd);
     free_program(pd->kv);
     free_program(pd->kv2);
-    for (auto& kv : pd->partial) free_program(kv.second);
-    for (auto& kv : pd->q_chunks) free_program(kv.second);
-    for (auto& kv : pd->kv_chunks) free_program(kv.second);
-    for (auto& kv : pd->kv2_chunks) free_program(kv.second);
+    for (auto& cache : pd->ranges)
+      for (auto& e : cache) { free_program(e.dev); if (e.ready) cudaEventDestroy(e.ready); }
+    if (switched) cudaSetDevice(cur);
     delete pd;
   }
   delete plan;
@@ -341,14 +439,13 @@ size_t sap_workspace_bytes(const sap_plan_t* plan, int n_q_heads, int n_kv_heads
 }
 
 int sap_attn_fwd(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev, sap_plan_t* plan,
-                 void* out, float* lse, int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
+                 int64_t n_tokens, void* out, float* lse, int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
                  void* workspace, size_t workspace_bytes, void* cuda_stream) {
   (void)workspace; (void)workspace_bytes;
   if (!q || !k || !v || !cu_seqlens_dev || !out || !lse) return SAP_ERR_INVALID_ARG;
-  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  int rc = check_call(plan, n_tokens, n_q_heads, n_kv_heads, head_dim, softmax_scale);
   if (rc != SAP_OK) return rc;
   if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out)) return SAP_ERR_UNSUPPORTED;
-  if ((rc = sap_plan_upload(plan)) != SAP_OK) return rc;
   const PlanDevice* pd = static_cast<const PlanDevice*>(plan->dev_state);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (head_dim == 128)
@@ -357,30 +454,32 @@ int sap_attn_fwd(const void* q, const void* k, const void* v, const int32_t* cu_
 }
 
 int sap_attn_fwd_partial(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev, sap_plan_t* plan,
-                         int32_t item_begin, int32_t item_end, float* out_f32, float* lse, int n_q_heads,
+                         int64_t n_tokens, int32_t item_begin, int32_t item_end, float* out_f32, float* lse, int n_q_heads,
                          int n_kv_heads, int head_dim, float softmax_scale, void* cuda_stream) {
   if (!q || !k || !v || !cu_seqlens_dev || !out_f32 || !lse) return SAP_ERR_INVALID_ARG;
-  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  int rc = check_call(plan, n_tokens, n_q_heads, n_kv_heads, head_dim, softmax_scale);
   if (rc != SAP_OK) return rc;
-  if (item_begin < 0 || item_end < item_begin || item_end > (int32_t)plan->items.size()) return SAP_ERR_INVALID_ARG;
+  if (!item_range_ok(plan, item_begin, item_end)) return SAP_ERR_INVALID_ARG;
   if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out_f32)) return SAP_ERR_UNSUPPORTED;
-  if ((rc = sap_plan_upload(plan)) != SAP_OK) return rc;
-  PlanDevice* pd = static_cast<PlanDevice*>(plan->dev_state);
-  DevProgram prog;
-  {
-    std::lock_guard<std::mutex> lock(plan->mu);
-    auto key = std::make_pair(item_begin, item_end);
-    auto itp = pd->partial.find(key);
-    if (itp == pd->partial.end()) {
-      TileProgram host;
-      build_q_program(*plan, item_begin, item_end, host);
-      DevProgram dp;
-      if ((rc = upload_program(host, dp)) != SAP_OK) return rc;
-      itp = pd->partial.emplace(key, dp).first;
-    }
-    prog = itp->second;
-  }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  DevProgram prog;
+  if ((rc = get_range_program(plan, kRangeItemsQ, item_begin, item_end, st, &prog)) != SAP_OK) return rc;
+  if (head_dim == 128)
+    return launch_fwd<128, true>(prog, q, k, v, cu_seqlens_dev, plan, nullptr, out_f32, lse, n_q_heads, n_kv_heads, softmax_scale, st);
+  return launch_fwd<64, true>(prog, q, k, v, cu_seqlens_dev, plan, nullptr, out_f32, lse, n_q_heads, n_kv_heads, softmax_scale, st);
+}
+
+int sap_attn_fwd_items(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev, sap_plan_t* plan,
+                       int64_t n_tokens, int32_t item_begin, int32_t item_end, float* out_f32, float* lse, int n_q_heads,
+                       int n_kv_heads, int head_dim, float softmax_scale, void* cuda_stream) {
+  if (!q || !k || !v || !cu_seqlens_dev || !out_f32 || !lse) return SAP_ERR_INVALID_ARG;
+  int rc = check_call(plan, n_tokens, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  if (rc != SAP_OK) return rc;
+  if (!item_range_ok(plan, item_begin, item_end)) return SAP_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out_f32)) return SAP_ERR_UNSUPPORTED;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  DevProgram prog;
+  if ((rc = get_range_program(plan, kRangeItemsQDrop, item_begin, item_end, st, &prog)) != SAP_OK) return rc;
   if (head_dim == 128)
     return launch_fwd<128, true>(prog, q, k, v, cu_seqlens_dev, plan, nullptr, out_f32, lse, n_q_heads, n_kv_heads, softmax_scale, st);
   return launch_fwd<64, true>(prog, q, k, v, cu_seqlens_dev, plan, nullptr, out_f32, lse, n_q_heads, n_kv_heads, softmax_scale, st);
@@ -393,7 +492,7 @@ int sap_lse_merge(const float* o_a, const float* lse_a, const float* o_b, const 
   if (n_tokens < 1 || n_q_heads < 1 || row_begin < 0 || row_end < row_begin || row_end > n_tokens) return SAP_ERR_INVALID_ARG;
   if (head_dim < 4 || head_dim % 4 != 0) return SAP_ERR_UNSUPPORTED;
   if (!aligned16(o_a) || !aligned16(o_b) || (reinterpret_cast<uintptr_t>(o_out) & 7u)) return SAP_ERR_UNSUPPORTED;
-  int rc = check_device_is_sm100();
+  int rc = ensure_device(nullptr);
   if (rc != SAP_OK) return rc;
   const int64_t n_rows = (row_end - row_begin) * n_q_heads;
   if (n_rows == 0) return SAP_OK;
@@ -412,23 +511,19 @@ int sap_lse_merge(const float* o_a, const float* lse_a, const float* o_b, const 
 }
 
 int sap_attn_bwd(const void* dout, const void* q, const void* k, const void* v, const void* out, const float* lse,
-                 const int32_t* cu_seqlens_dev, sap_plan_t* plan, void* dq, void* dk, void* dv, int n_q_heads,
+                 const int32_t* cu_seqlens_dev, sap_plan_t* plan, int64_t n_tokens, void* dq, void* dk, void* dv, int n_q_heads,
                  int n_kv_heads, int head_dim, float softmax_scale, void* workspace, size_t workspace_bytes,
                  void* cuda_stream) {
   if (!dout || !q || !k || !v || !out || !lse || !cu_seqlens_dev || !dq || !dk || !dv) return SAP_ERR_INVALID_ARG;
-  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  int rc = check_call(plan, n_tokens, n_q_heads, n_kv_heads, head_dim, softmax_scale);
   if (rc != SAP_OK) return rc;
   if (!aligned16(dout) || !aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out) || !aligned16(dq) ||
-      !aligned16(dk) || !aligned16(dv) || !aligned16(workspace))
+      !aligned16(dk) || !aligned16(dv))
     return SAP_ERR_UNSUPPORTED;
-  const size_t need = sap_workspace_bytes(plan, n_q_heads, n_kv_heads, head_dim, SAP_PASS_BWD);
-  if (!workspace || workspace_bytes < need) return SAP_ERR_WORKSPACE_TOO_SMALL;
-  if ((rc = sap_plan_upload(plan)) != SAP_OK) return rc;
+  float *dsum, *dq_acc;
+  if ((rc = bwd_ws(plan, n_q_heads, n_kv_heads, head_dim, workspace, workspace_bytes, &dsum, &dq_acc)) != SAP_OK) return rc;
   const PlanDevice* pd = static_cast<const PlanDevice*>(plan->dev_state);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  float* dsum = static_cast<float*>(workspace);
-  float* dq_acc = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) +
-                                           align256(static_cast<size_t>(plan->n_tokens) * n_q_heads * sizeof(float)));
   if (head_dim == 128)
     return launch_bwd<128>(pd, dout, q, k, v, out, lse, cu_seqlens_dev, plan, dq, dk, dv, n_q_heads, n_kv_heads,
                            softmax_scale, dsum, dq_acc, st);
@@ -437,85 +532,109 @@ int sap_attn_bwd(const void* dout, const void* q, const void* k, const void* v, 
 }
 
 int sap_attn_fwd_chunks(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev, sap_plan_t* plan,
-                        int32_t q_chunk_begin, int32_t q_chunk_end, void* out, float* lse, int n_q_heads, int n_kv_heads,
-                        int head_dim, float softmax_scale, void* cuda_stream) {
+                        int64_t n_tokens, int32_t q_chunk_begin, int32_t q_chunk_end, void* out, float* lse, int n_q_heads,
+                        int n_kv_heads, int head_dim, float softmax_scale, void* cuda_stream) {
   if (!q || !k || !v || !cu_seqlens_dev || !out || !lse) return SAP_ERR_INVALID_ARG;
-  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  int rc = check_call(plan, n_tokens, n_q_heads, n_kv_heads, head_dim, softmax_scale);
   if (rc != SAP_OK) return rc;
   if (!chunk_range_ok(plan, q_chunk_begin, q_chunk_end)) return SAP_ERR_INVALID_ARG;
   if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out)) return SAP_ERR_UNSUPPORTED;
-  if ((rc = sap_plan_upload(plan)) != SAP_OK) return rc;
   if (q_chunk_begin == q_chunk_end) return SAP_OK;
-  DevProgram prog;
-  if ((rc = get_chunk_program(plan, 0, q_chunk_begin, q_chunk_end, &prog)) != SAP_OK) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  DevProgram prog;
+  if ((rc = get_range_program(plan, kRangeQ, q_chunk_begin, q_chunk_end, st, &prog)) != SAP_OK) return rc;
   if (head_dim == 128)
     return launch_fwd<128, false>(prog, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st);
   return launch_fwd<64, false>(prog, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st);
 }
 
-static int bwd_ws(const sap_plan_t* plan, int Hq, int Hkv, int d, void* workspace, size_t bytes, float** dsum, float** dq_acc) {
-  if (!aligned16(workspace)) return SAP_ERR_UNSUPPORTED;
-  if (!workspace || bytes < sap_workspace_bytes(plan, Hq, Hkv, d, SAP_PASS_BWD)) return SAP_ERR_WORKSPACE_TOO_SMALL;
-  *dsum = static_cast<float*>(workspace);
-  *dq_acc = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + align256(static_cast<size_t>(plan->n_tokens) * Hq * sizeof(float)));
-  return SAP_OK;
-}
-
-int sap_attn_bwd_begin(const void* dout, const void* out, sap_plan_t* plan, int32_t q_chunk_begin, int32_t q_chunk_end,
-                       int n_q_heads, int n_kv_heads, int head_dim, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+int sap_attn_bwd_begin(const void* dout, const void* out, sap_plan_t* plan, int64_t n_tokens, int32_t q_chunk_begin,
+                       int32_t q_chunk_end, int n_q_heads, int n_kv_heads, int head_dim, void* workspace,
+                       size_t workspace_bytes, void* cuda_stream) {
   if (!dout || !out) return SAP_ERR_INVALID_ARG;
-  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, 1.f);
+  int rc = check_call(plan, n_tokens, n_q_heads, n_kv_heads, head_dim, 1.f, /*need_upload=*/false);
   if (rc != SAP_OK) return rc;
   if (!chunk_range_ok(plan, q_chunk_begin, q_chunk_end)) return SAP_ERR_INVALID_ARG;
   if (!aligned16(dout) || !aligned16(out)) return SAP_ERR_UNSUPPORTED;
   float *dsum, *dq_acc;
   if ((rc = bwd_ws(plan, n_q_heads, n_kv_heads, head_dim, workspace, workspace_bytes, &dsum, &dq_acc)) != SAP_OK) return rc;
-  if ((rc = check_device_is_sm100()) != SAP_OK) return rc;
   const int64_t t0 = (int64_t)q_chunk_begin * plan->chunk_len, nt = (int64_t)(q_chunk_end - q_chunk_begin) * plan->chunk_len;
-  if (nt == 0) return SAP_OK;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  if (head_dim == 128) return launch_bwd_begin<128>(dout, out, plan->n_tokens, n_q_heads, t0, nt, dsum, dq_acc, st);
-  return launch_bwd_begin<64>(dout, out, plan->n_tokens, n_q_heads, t0, nt, dsum, dq_acc, st);
+  if (head_dim == 128) return launch_bwd_pre<128>(dout, out, plan->n_tokens, n_q_heads, t0, nt, dsum, dq_acc, true, st);
+  return launch_bwd_pre<64>(dout, out, plan->n_tokens, n_q_heads, t0, nt, dsum, dq_acc, true, st);
+}
+
+// shared tail of sap_attn_bwd_chunks / sap_attn_bwd_items
+static int bwd_range(int kind1, int kind2, int32_t a, int32_t b, const void* dout, const void* q, const void* k, const void* v,
+                     const float* lse, const int32_t* cu, sap_plan_t* plan, void* dk, void* dv, int Hq, int Hkv, int d,
+                     float scale, void* workspace, size_t workspace_bytes, cudaStream_t st) {
+  if (!aligned16(dout) || !aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(dk) || !aligned16(dv)) return SAP_ERR_UNSUPPORTED;
+  float *dsum, *dq_acc;
+  int rc;
+  if ((rc = bwd_ws(plan, Hq, Hkv, d, workspace, workspace_bytes, &dsum, &dq_acc)) != SAP_OK) return rc;
+  if (a == b) return SAP_OK;
+  DevProgram prog;
+  if ((rc = get_range_program(plan, use_pair_kernel(d) ? kind2 : kind1, a, b, st, &prog)) != SAP_OK) return rc;
+  if (d == 128) return launch_bwd_main<128>(prog, prog, dout, q, k, v, lse, cu, plan, dk, dv, Hq, Hkv, scale, dsum, dq_acc, st);
+  return launch_bwd_main<64>(prog, prog, dout, q, k, v, lse, cu, plan, dk, dv, Hq, Hkv, scale, dsum, dq_acc, st);
 }
 
 int sap_attn_bwd_chunks(const void* dout, const void* q, const void* k, const void* v, const float* lse,
-                        const int32_t* cu_seqlens_dev, sap_plan_t* plan, int32_t kv_chunk_begin, int32_t kv_chunk_end,
-                        void* dk, void* dv, int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
-                        void* workspace, size_t workspace_bytes, void* cuda_stream) {
+                        const int32_t* cu_seqlens_dev, sap_plan_t* plan, int64_t n_tokens, int32_t kv_chunk_begin,
+                        int32_t kv_chunk_end, void* dk, void* dv, int n_q_heads, int n_kv_heads, int head_dim,
+                        float softmax_scale, void* workspace, size_t workspace_bytes, void* cuda_stream) {
   if (!dout || !q || !k || !v || !lse || !cu_seqlens_dev || !dk || !dv) return SAP_ERR_INVALID_ARG;
-  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  int rc = check_call(plan, n_tokens, n_q_heads, n_kv_heads, head_dim, softmax_scale);
   if (rc != SAP_OK) return rc;
   if (!chunk_range_ok(plan, kv_chunk_begin, kv_chunk_end)) return SAP_ERR_INVALID_ARG;
   if (plan->chunk_len % kTile != 0) return SAP_ERR_UNSUPPORTED;  // K/V tiles must not straddle two ranks' chunks
-  if (!aligned16(dout) || !aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(dk) || !aligned16(dv)) return SAP_ERR_UNSUPPORTED;
-  float *dsum, *dq_acc;
-  if ((rc = bwd_ws(plan, n_q_heads, n_kv_heads, head_dim, workspace, workspace_bytes, &dsum, &dq_acc)) != SAP_OK) return rc;
-  if ((rc = sap_plan_upload(plan)) != SAP_OK) return rc;
-  if (kv_chunk_begin == kv_chunk_end) return SAP_OK;
-  const bool pair = head_dim == 128 && g_bwd_form.load() == 0;
-  DevProgram prog;
-  if ((rc = get_chunk_program(plan, pair ? 2 : 1, kv_chunk_begin, kv_chunk_end, &prog)) != SAP_OK) return rc;
-  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  if (head_dim == 128)
-    return launch_bwd_main<128>(prog, prog, dout, q, k, v, lse, cu_seqlens_dev, plan, dk, dv, n_q_heads, n_kv_heads,
-                                softmax_scale, dsum, dq_acc, st);
-  return launch_bwd_main<64>(prog, prog, dout, q, k, v, lse, cu_seqlens_dev, plan, dk, dv, n_q_heads, n_kv_heads,
-                             softmax_scale, dsum, dq_acc, st);
+  return bwd_range(kRangeKv, kRangeKvPair, kv_chunk_begin, kv_chunk_end, dout, q, k, v, lse, cu_seqlens_dev, plan, dk, dv,
+                   n_q_heads, n_kv_heads, head_dim, softmax_scale, workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
 }
 
-int sap_attn_bwd_end(sap_plan_t* plan, int32_t q_chunk_begin, int32_t q_chunk_end, void* dq, int n_q_heads, int n_kv_heads,
-                     int head_dim, float softmax_scale, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+int sap_attn_bwd_items(const void* dout, const void* q, const void* k, const void* v, const float* lse,
+                       const int32_t* cu_seqlens_dev, sap_plan_t* plan, int64_t n_tokens, int32_t item_begin,
+                       int32_t item_end, void* dk, void* dv, int n_q_heads, int n_kv_heads, int head_dim,
+                       float softmax_scale, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!dout || !q || !k || !v || !lse || !cu_seqlens_dev || !dk || !dv) return SAP_ERR_INVALID_ARG;
+  int rc = check_call(plan, n_tokens, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  if (rc != SAP_OK) return rc;
+  if (!item_range_ok(plan, item_begin, item_end)) return SAP_ERR_INVALID_ARG;
+  return bwd_range(kRangeItemsKv, kRangeItemsKvPair, item_begin, item_end, dout, q, k, v, lse, cu_seqlens_dev, plan, dk, dv,
+                   n_q_heads, n_kv_heads, head_dim, softmax_scale, workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int sap_attn_bwd_end(sap_plan_t* plan, int64_t n_tokens, int32_t q_chunk_begin, int32_t q_chunk_end, void* dq, int n_q_heads,
+                     int n_kv_heads, int head_dim, float softmax_scale, void* workspace, size_t workspace_bytes,
+                     void* cuda_stream) {
   if (!dq) return SAP_ERR_INVALID_ARG;
-  int rc = check_dims(plan, n_q_heads, n_kv_heads, head_dim, softmax_scale);
+  int rc = check_call(plan, n_tokens, n_q_heads, n_kv_heads, head_dim, softmax_scale, /*need_upload=*/false);
   if (rc != SAP_OK) return rc;
   if (!chunk_range_ok(plan, q_chunk_begin, q_chunk_end)) return SAP_ERR_INVALID_ARG;
   if (!aligned16(dq)) return SAP_ERR_UNSUPPORTED;
   float *dsum, *dq_acc;
   if ((rc = bwd_ws(plan, n_q_heads, n_kv_heads, head_dim, workspace, workspace_bytes, &dsum, &dq_acc)) != SAP_OK) return rc;
-  if ((rc = check_device_is_sm100()) != SAP_OK) return rc;
   const int64_t t0 = (int64_t)q_chunk_begin * plan->chunk_len, nt = (int64_t)(q_chunk_end - q_chunk_begin) * plan->chunk_len;
-  return launch_bwd_end(dq_acc, dq, n_q_heads, head_dim, t0, nt, softmax_scale, static_cast<cudaStream_t>(cuda_stream));
+  return launch_bwd_post(dq_acc, dq, n_q_heads, head_dim, t0, nt, softmax_scale, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int sap_axpy(void* dst, int dst_is_bf16, const void* src, int src_is_bf16, int64_t n_elems, float alpha, int accumulate,
+             void* cuda_stream) {
+  if (!dst || !src || n_elems < 0) return SAP_ERR_INVALID_ARG;
+  if (n_elems % 8 != 0 || !aligned16(dst) || !aligned16(src)) return SAP_ERR_UNSUPPORTED;
+  int rc = ensure_device(nullptr);
+  if (rc != SAP_OK) return rc;
+  if (n_elems == 0) return SAP_OK;
+  const int64_t n8 = n_elems / 8, want = (n8 + 255) / 256;
+  const unsigned grid = static_cast<unsigned>(want < 148 * 16 ? want : 148 * 16);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (dst_is_bf16 && src_is_bf16) sap_axpy_kernel<true, true><<<grid, 256, 0, st>>>(dst, src, n8, alpha, accumulate);
+  else if (dst_is_bf16) sap_axpy_kernel<true, false><<<grid, 256, 0, st>>>(dst, src, n8, alpha, accumulate);
+  else if (src_is_bf16) sap_axpy_kernel<false, true><<<grid, 256, 0, st>>>(dst, src, n8, alpha, accumulate);
+  else sap_axpy_kernel<false, false><<<grid, 256, 0, st>>>(dst, src, n8, alpha, accumulate);
+  g_launch_count.fetch_add(1);
+  SAP_CUDA_CHECK(cudaGetLastError());
+  return SAP_OK;
 }
 
 }  // extern "C"

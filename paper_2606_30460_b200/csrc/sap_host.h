@@ -4,7 +4,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <atomic>
-#include <map>
+#include <list>
 #include <utility>
 #include "sap_internal.h"
 
@@ -28,16 +28,27 @@ struct DevProgram {
   int32_t n_tiles = 0;
 };
 
-// Device copies owned by a plan (freed by sap_plan_destroy).
+// A range-restricted program (partial forward over an item range, per-rank launches over a chunk range, per-item
+// backward): built on first use, uploaded on the caller's stream, kept with the plan.
+struct RangeProgram {
+  std::pair<int32_t, int32_t> key;
+  TileProgram host;            // source of the asynchronous upload; must outlive it
+  DevProgram dev;
+  cudaEvent_t ready = nullptr; // recorded behind the upload: other streams wait on it
+  cudaStream_t stream = nullptr;
+};
+enum { kRangeItemsQ = 0, kRangeQ = 1, kRangeKv = 2, kRangeKvPair = 3, kRangeItemsKv = 4, kRangeItemsKvPair = 5, kRangeItemsQDrop = 6, kRangeKinds = 7 };
+
+// Device copies owned by a plan (freed by sap_plan_destroy).  A plan's mirror lives on ONE device (the current
+// device of the first upload); calls with another current device return SAP_ERR_PLAN_MISMATCH.
 struct PlanDevice {
   bool uploaded = false;
   int device = -1;
   DevProgram fwd, kv, kv2;
-  std::map<std::pair<int32_t, int32_t>, DevProgram> partial;  // item-range-restricted Q programs
-  std::map<std::pair<int32_t, int32_t>, DevProgram> q_chunks, kv_chunks, kv2_chunks;  // chunk-range-restricted programs (per-rank launches)
+  std::list<RangeProgram> ranges[kRangeKinds];   // most recently used first
 };
 
-int check_device_is_sm100();
+int ensure_device(int* dev_out);
 int upload_program(const TileProgram& host, DevProgram& dev);
 void free_program(DevProgram& dev);
 

@@ -55,5 +55,7 @@ namespace sap {
 // `drop_empty`: leave out tiles that have no work among those items (a rank's launch touches only its own rows).
 void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, TileProgram& out, bool drop_empty = false);
 // K/V tiles of kv-chunks [chunk_begin, chunk_end) only (the whole sequence by default).
-void build_kv_program(const sap_plan& p, TileProgram& out, int32_t chunk_begin = 0, int32_t chunk_end = -1, int32_t tile_rows = kTile);
+// `item_begin..item_end` keeps only segments of those plan items; `drop_empty` leaves out tiles without work.
+void build_kv_program(const sap_plan& p, TileProgram& out, int32_t chunk_begin = 0, int32_t chunk_end = -1, int32_t tile_rows = kTile,
+                      int32_t item_begin = 0, int32_t item_end = -1, bool drop_empty = false);
 }  // namespace sap

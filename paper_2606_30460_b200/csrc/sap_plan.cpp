@@ -75,7 +75,9 @@ void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, Ti
   out.tiles.swap(sorted);
 }
 
-void build_kv_program(const sap_plan& p, TileProgram& out, int32_t chunk_begin, int32_t chunk_end, int32_t tile_rows) {
+void build_kv_program(const sap_plan& p, TileProgram& out, int32_t chunk_begin, int32_t chunk_end, int32_t tile_rows,
+                      int32_t item_begin, int32_t item_end, bool drop_empty) {
+  if (item_end < 0) item_end = (int32_t)p.items.size();
   out.tiles.clear();
   out.segs.clear();
   out.streamed_tiles = 0;
@@ -96,6 +98,7 @@ void build_kv_program(const sap_plan& p, TileProgram& out, int32_t chunk_begin, 
     for (int32_t j = j_lo; j <= j_hi; ++j) {
       for (int32_t x = p.kv_offsets[j]; x < p.kv_offsets[j + 1]; ++x) {
         const int32_t it = p.kv_index[x];
+        if (it < item_begin || it >= item_end) continue;
         const sap_item_t& im = p.items[it];
         const int64_t ca = std::max<int64_t>(c0, im.kv_begin), cb = std::min<int64_t>(c1, im.kv_end);
         if (ca >= cb) continue;
@@ -114,6 +117,7 @@ void build_kv_program(const sap_plan& p, TileProgram& out, int32_t chunk_begin, 
       }
     }
     td.seg_end = (int32_t)out.segs.size();
+    if (drop_empty && td.seg_end == td.seg_begin) continue;
     out.tiles.push_back(td);
     work.push_back(w);
     out.streamed_tiles += w;
@@ -350,6 +354,7 @@ const char* sap_strerror(int status) {
     case SAP_ERR_WRONG_ARCH: return "device is not sm_100 (B200)";
     case SAP_ERR_CUDA: return "CUDA error (see sap_last_cuda_error)";
     case SAP_ERR_NO_DEVICE: return "no CUDA device";
+    case SAP_ERR_PLAN_MISMATCH: return "plan mismatch (n_tokens differs from the plan's, or the plan lives on another device)";
     default: return "unknown status";
   }
 }

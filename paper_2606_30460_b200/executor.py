@@ -32,6 +32,8 @@ def sap_execute_fwd(q_shard, kv_shard, plan: Plan, slots: np.ndarray, rank: int,
 
     codes = plan.codegen(slots, rank)
     items = plan.items
+    # `rank` and the peers in the code list are ranks inside `group`; P2POp wants global ranks
+    glob = (lambda r: r) if group is None else (lambda r: dist.get_global_rank(group, r))
     stages = sorted(set(int(c[0]) for c in codes))
     q_buf, kv_buf, results, acc = {}, {}, {}, None           # per item: received q / kv; computed partials to send
     for st in stages:
@@ -40,11 +42,11 @@ def sap_execute_fwd(q_shard, kv_shard, plan: Plan, slots: np.ndarray, rank: int,
         for _, op, tensor, peer, item in (tuple(int(v) for v in c) for c in mine):
             if op == SAP_OP_SEND:
                 payload = q_shard if tensor == SAP_T_Q else kv_shard if tensor == SAP_T_KV else pack_o(*results.pop(item))
-                ops.append(dist.P2POp(dist.isend, payload.contiguous(), peer, group))
+                ops.append(dist.P2POp(dist.isend, payload.contiguous(), glob(peer), group))
             elif op == SAP_OP_RECV:
                 like = q_shard if tensor == SAP_T_Q else kv_shard if tensor == SAP_T_KV else o_template
                 recv[(tensor, peer, item)] = torch.empty_like(like)
-                ops.append(dist.P2POp(dist.irecv, recv[(tensor, peer, item)], peer, group))
+                ops.append(dist.P2POp(dist.irecv, recv[(tensor, peer, item)], glob(peer), group))
         reqs = dist.batch_isend_irecv(ops) if ops else []      # one batch per stage, in flight during the computing code
         for _, op, tensor, peer, item in (tuple(int(v) for v in c) for c in mine):
             if op != SAP_OP_COMPUTING:
@@ -75,20 +77,25 @@ def sap_execute_fwd(q_shard, kv_shard, plan: Plan, slots: np.ndarray, rank: int,
 
 
 
-def sap_execute_bwd(q_shard, do_pack, kv_shard, plan: Plan, slots: np.ndarray, rank: int, bwd_fn: Callable, group=None):
+def sap_execute_bwd(q_shard, do_pack, kv_shard, plan: Plan, slots: np.ndarray, rank: int, bwd_fn: Callable, group=None,
+                    add_fn: Callable = None):
     """Replays rank `rank`'s backward code list (sap_plan_codegen_bwd).  q_shard [n,Hq,d]; do_pack: this rank's dO
     rows with their LSE and D packed in one tensor (it travels as the `do` tensor of Table 1); kv_shard [2,n,Hkv,d].
     bwd_fn(item, q_shard, do_pack, kv_shard) -> (dq [n,Hq,d], dkv [2,n,Hkv,d]) : the item's contributions to the rows
     of chunk q_chunk(item) and to the keys of chunk kv_chunk(item), as tensors torch.distributed can send.
+    add_fn(acc, t) adds a contribution into a gradient in place (COPY of a received dq / dkv, Table 1); the default is
+    the tensor library's add for the CPU schedule tests, on a GPU pass api.sap_axpy (LocalExecutor does).
     Returns this rank's (dq, dkv): own contributions plus everything the COPY codes added."""
     import torch
     import torch.distributed as dist
 
     codes = plan.codegen(slots, rank, backward=True)
     items = plan.items
+    glob = (lambda r: r) if group is None else (lambda r: dist.get_global_rank(group, r))
     dq_acc, dkv_acc = None, None
     bufs, results = {}, {}                      # (tensor, item) -> received operand; (tensor, item) -> contribution to send
-    add = lambda acc, t: t.clone() if acc is None else acc + t
+    add_fn = add_fn or (lambda acc, t: acc.add_(t))
+    add = lambda acc, t: t.clone() if acc is None else add_fn(acc, t)
     for st in sorted(set(int(c[0]) for c in codes)):
         mine = [tuple(int(v) for v in c) for c in codes if int(c[0]) == st]
         ops, recv = [], {}
@@ -97,11 +104,11 @@ def sap_execute_bwd(q_shard, do_pack, kv_shard, plan: Plan, slots: np.ndarray, r
                 payload = {SAP_T_Q: q_shard, SAP_T_DO: do_pack, SAP_T_KV: kv_shard}.get(tensor)
                 if payload is None:
                     payload = results.pop((tensor, item))
-                ops.append(dist.P2POp(dist.isend, payload.contiguous(), peer, group))
+                ops.append(dist.P2POp(dist.isend, payload.contiguous(), glob(peer), group))
             elif op == SAP_OP_RECV:
                 like = {SAP_T_Q: q_shard, SAP_T_DO: do_pack, SAP_T_KV: kv_shard, SAP_T_DQ: q_shard, SAP_T_DKV: kv_shard}[tensor]
                 recv[(tensor, item)] = torch.empty_like(like)
-                ops.append(dist.P2POp(dist.irecv, recv[(tensor, item)], peer, group))
+                ops.append(dist.P2POp(dist.irecv, recv[(tensor, item)], glob(peer), group))
         reqs = dist.batch_isend_irecv(ops) if ops else []
         for _, op, tensor, peer, item in mine:
             if op != SAP_OP_COMPUTING:
@@ -133,3 +140,254 @@ def sap_execute_bwd(q_shard, do_pack, kv_shard, plan: Plan, slots: np.ndarray, r
                 bufs[(tensor, item)] = buf
     assert not bufs and not results, "every transferred tensor was consumed"
     return dq_acc, dkv_acc
+
+
+# ======================================================================================================================
+# One-GPU replay: the P ranks are emulated in one process (BASELINE.json north_star: "the P ranks are emulated as P
+# sequence chunks in HBM"), every rank's code list is executed stage by stage, the transport is a device copy into the
+# receiver's staging buffer, and every arithmetic step is a kernel behind the C ABI.
+# ======================================================================================================================
+class ShardView:
+    """A shard [n, H, d] that the kernels address with GLOBAL token indices: data_ptr() is moved back by `row0` rows,
+    so that row t of the whole tensor lands on row t - row0 of the shard.  The kernels touch only the rows their tile
+    program names (the shard's), so a rank needs memory for one shard, not for the sequence."""
+
+    def __init__(self, shard, row0: int, n_tokens: int):
+        assert shard.is_contiguous()
+        self._t, self._row0 = shard, int(row0)
+        self.shape = (int(n_tokens),) + tuple(shard.shape[1:])
+        self.dtype, self.device, self.is_cuda = shard.dtype, shard.device, shard.is_cuda
+
+    def is_contiguous(self):
+        return True
+
+    def data_ptr(self):
+        return self._t.data_ptr() - self._row0 * self._t.stride(0) * self._t.element_size()
+
+
+def _max_inflight(code_lists, tensor_kinds):
+    """largest number of same-kind RECVs one rank has in one stage: the 'fixed multiple' of a shard the staging area
+    needs (PAPER.md:140)"""
+    worst = 1
+    for codes in code_lists:
+        count = {}
+        for st, op, tensor, peer, item in codes.tolist():
+            if op == SAP_OP_RECV and tensor in tensor_kinds:
+                count[(st, tensor)] = count.get((st, tensor), 0) + 1
+        worst = max([worst] + list(count.values()))
+    return worst
+
+
+class LocalExecutor:
+    """Replays the jitted code lists of all P ranks on ONE GPU (forward and backward).
+
+    Per rank: its own shards (views of the caller's tensors), one compute buffer per operand kind (q, kv, do) that COPY
+    fills from the staging area ("copy from the communication buffer to the compute buffer"), a staging
+    area of a fixed number of shard-sized slots per tensor kind allocated ONCE (:140-142), and the running result.
+    SEND / RECV of a stage are matched across ranks and executed as device copies before the stage's COMPUTING codes,
+    COPY codes after them, exactly in the order of the lists (sap_plan_codegen / sap_plan_codegen_bwd).  COMPUTING
+    asserts that its operands are present: an illegal schedule fails here, not in the numerics."""
+
+    def __init__(self, plan: Plan, slots: np.ndarray, n_q_heads: int, n_kv_heads: int, head_dim: int, device,
+                 softmax_scale=None):
+        import torch
+        self.plan, self.slots = plan, np.ascontiguousarray(slots, dtype=np.int32)
+        self.P, self.N = plan.n_chunks, plan.n_tokens
+        self.n = self.N // self.P
+        self.Hq, self.Hkv, self.d, self.dev = n_q_heads, n_kv_heads, head_dim, device
+        self.scale = float(head_dim) ** -0.5 if softmax_scale is None else float(softmax_scale)
+        self.items = plan.items
+        # K/V tiles of the per-item backward are 256 keys (head_dim 128) or 128 keys wide from token 0: a rank's shard-sized
+        # dK / dV buffer holds whole tiles only if the chunk length is a multiple of that
+        assert self.n % (256 if head_dim == 128 else 128) == 0, "chunk length must be a multiple of the K/V tile"
+        self.fwd_codes = [plan.codegen(self.slots, r) for r in range(self.P)]
+        self.bwd_codes = [plan.codegen(self.slots, r, backward=True) for r in range(self.P)]
+        n, Hq, Hkv, d, P = self.n, n_q_heads, n_kv_heads, head_dim, self.P
+        bf, f32 = torch.bfloat16, torch.float32
+        e = lambda *shape, dtype=bf: torch.empty(shape, dtype=dtype, device=device)
+        kq = _max_inflight(self.fwd_codes + self.bwd_codes, (SAP_T_Q,))
+        kkv = _max_inflight(self.fwd_codes + self.bwd_codes, (SAP_T_KV,))
+        ko = _max_inflight(self.fwd_codes, (SAP_T_O,))
+        kdo = _max_inflight(self.bwd_codes, (SAP_T_DO,))
+        kdq = _max_inflight(self.bwd_codes, (SAP_T_DQ,))
+        kdkv = _max_inflight(self.bwd_codes, (SAP_T_DKV,))
+        self.staging_slots = {"q": kq, "kv": kkv, "o": ko, "do": kdo, "dq": kdq, "dkv": kdkv}
+        # fixed buffers, allocated once for all P emulated ranks (one of each per rank)
+        self.stage_q = e(P, kq, n, Hq, d); self.stage_kv = e(P, kkv, 2, n, Hkv, d)
+        self.stage_o = e(P, ko, n, Hq, d, dtype=f32); self.stage_ol = e(P, ko, Hq, n, dtype=f32)
+        self.stage_do = e(P, kdo, n, Hq, d); self.stage_dol = e(P, kdo, 2, Hq, n, dtype=f32)      # dO with LSE and D
+        self.stage_dq = e(P, kdq, n, Hq, d, dtype=f32); self.stage_dkv = e(P, kdkv, 2, n, Hkv, d)
+        self.comp_q = e(P, n, Hq, d); self.comp_kv = e(P, 2, n, Hkv, d)
+        self.comp_do = e(P, n, Hq, d); self.comp_dol = e(P, 2, Hq, n, dtype=f32)
+        self.part_o = e(n, Hq, d, dtype=f32); self.part_l = e(Hq, self.N, dtype=f32)              # one partial result
+        self.scratch_dkv = e(2, n, Hkv, d)
+
+    # ------------------------------------------------------------------------------------------------ helpers
+    def _walk(self, code_lists, on_transfer, on_compute, on_copy):
+        stages = sorted(set(int(c[0]) for codes in code_lists for c in codes))
+        for st in stages:
+            per_rank = [[tuple(int(v) for v in c) for c in codes if int(c[0]) == st] for codes in code_lists]
+            sends = {(tensor, r, peer, item) for r, mine in enumerate(per_rank) for _, op, tensor, peer, item in mine if op == SAP_OP_SEND}
+            recvs = [(tensor, peer, r, item) for r, mine in enumerate(per_rank) for _, op, tensor, peer, item in mine if op == SAP_OP_RECV]
+            assert sends == set(recvs) and len(recvs) == len(set(recvs)), f"stage {st}: SEND / RECV codes do not pair up"
+            slot_of = {}
+            for tensor, src, dst, item in recvs:                    # the batched isend/irecv of the stage
+                k = sum(1 for (t2, _, d2, _) in slot_of if t2 == tensor and d2 == dst)
+                slot_of[(tensor, src, dst, item)] = k
+                on_transfer(tensor, src, dst, item, k)
+            for r, mine in enumerate(per_rank):
+                for _, op, tensor, peer, item in mine:
+                    if op == SAP_OP_COMPUTING:
+                        on_compute(r, item)
+            for r, mine in enumerate(per_rank):
+                for _, op, tensor, peer, item in mine:
+                    if op == SAP_OP_COPY:
+                        on_copy(r, tensor, peer, item, slot_of[(tensor, peer, r, item)])
+
+    # ------------------------------------------------------------------------------------------------ forward
+    def forward(self, q, k, v, cu_seqlens_dev):
+        """q [N,Hq,d], k, v [N,Hkv,d] bf16 on the device (rank r owns rows [r n, (r+1) n)).  Returns out bf16 [N,Hq,d],
+        lse fp32 [Hq,N]."""
+        import torch
+        from . import api
+        n, N, P, Hq = self.n, self.N, self.P, self.Hq
+        own_q = lambda r: q[r * n:(r + 1) * n]
+        own_kv = lambda r: (k[r * n:(r + 1) * n], v[r * n:(r + 1) * n])
+        acc_o = torch.zeros((P, n, Hq, self.d), dtype=torch.float32, device=self.dev)
+        acc_l = torch.full((P, Hq, n), float("-inf"), dtype=torch.float32, device=self.dev)
+        have_q, have_kv, results = {}, {}, {}      # (rank, item) -> operand in the compute buffer; helper partials
+
+        def merge(r, item, o, l):
+            # only the 128-row Q tiles the item touches hold a partial result (sap_attn_fwd_items leaves the others alone)
+            rb = (int(self.items[item, 6]) - r * n) // 128 * 128
+            re = min(n, -(-(int(self.items[item, 7]) - r * n) // 128) * 128)
+            api.sap_lse_merge(acc_o[r], acc_l[r], o, l, row_begin=rb, row_end=re, o_out=acc_o[r], lse_out=acc_l[r])
+
+        def on_transfer(tensor, src, dst, item, slot):
+            if tensor == SAP_T_Q:
+                self.stage_q[dst, slot].copy_(own_q(src))
+            elif tensor == SAP_T_KV:
+                kk, vv = own_kv(src)
+                self.stage_kv[dst, slot, 0].copy_(kk); self.stage_kv[dst, slot, 1].copy_(vv)
+            else:
+                o, l = results.pop((src, item))
+                self.stage_o[dst, slot].copy_(o); self.stage_ol[dst, slot].copy_(l)
+
+        def on_compute(r, item):
+            i, j = int(self.items[item, 0]), int(self.items[item, 1])
+            assert r in (i, j)
+            if i == r:
+                qs = own_q(r)
+            else:
+                assert have_q.pop((r, item), False), f"rank {r}: Q of item {item} is not in the compute buffer"
+                qs = self.comp_q[r]
+            if j == r:
+                ks, vs = own_kv(r)
+            else:
+                assert have_kv.pop((r, item), False), f"rank {r}: K/V of item {item} is not in the compute buffer"
+                ks, vs = self.comp_kv[r, 0], self.comp_kv[r, 1]
+            qg, kg, vg = ShardView(qs.contiguous(), i * n, N), ShardView(ks.contiguous(), j * n, N), ShardView(vs.contiguous(), j * n, N)
+            api.sap_attn_fwd_items(qg, kg, vg, cu_seqlens_dev, self.plan, item, item + 1, ShardView(self.part_o, i * n, N),
+                                          self.part_l, Hq, self.Hkv, self.d, softmax_scale=self.scale)
+            o, l = self.part_o, self.part_l[:, i * n:(i + 1) * n].contiguous()
+            if i == r:
+                merge(r, item, o, l)
+            else:
+                results[(r, item)] = (o.clone(), l)          # a helper's partial: travels back one stage later
+
+        def on_copy(r, tensor, peer, item, slot):
+            if tensor == SAP_T_Q:
+                self.comp_q[r].copy_(self.stage_q[r, slot]); have_q[(r, item)] = True
+            elif tensor == SAP_T_KV:
+                self.comp_kv[r].copy_(self.stage_kv[r, slot]); have_kv[(r, item)] = True
+            else:                                            # copy and rescale
+                merge(r, item, self.stage_o[r, slot], self.stage_ol[r, slot])
+
+        self._walk(self.fwd_codes, on_transfer, on_compute, on_copy)
+        assert not have_q and not have_kv and not results, "every transferred tensor was consumed"
+        out = torch.empty_like(q)
+        api.sap_axpy(out, acc_o.reshape(N, Hq, self.d), 1.0, accumulate=False)
+        return out, acc_l.permute(1, 0, 2).reshape(Hq, N).contiguous()
+
+    # ------------------------------------------------------------------------------------------------ backward
+    def backward(self, dout, q, k, v, out, lse, cu_seqlens_dev):
+        """Returns dq [N,Hq,d], dk, dv [N,Hkv,d] bf16."""
+        import torch
+        from . import api
+        n, N, P, Hq, Hkv, d = self.n, self.N, self.P, self.Hq, self.Hkv, self.d
+        need = api.sap_workspace_bytes(self.plan, Hq, Hkv, d, 1)
+        ws_own = torch.empty(need, dtype=torch.uint8, device=self.dev)    # owners' D and dQ accumulator rows
+        ws_help = torch.empty(need, dtype=torch.uint8, device=self.dev)   # scratch of the rank that helps another
+        acc_off = ((N * Hq * 4 + 255) // 256) * 256
+        dsum = lambda ws: ws[:N * Hq * 4].view(torch.float32).view(Hq, N)
+        dqacc = lambda ws: ws[acc_off:acc_off + N * Hq * d * 4].view(torch.float32).view(N, Hq, d)
+        for r in range(P):   # every rank: D of its rows, zero its accumulator rows (sap_attn_bwd_begin)
+            api.sap_attn_bwd_begin(dout, out, self.plan, r, r + 1, Hkv, ws_own)
+        dkv_tot = torch.zeros((2, N, Hkv, d), dtype=torch.float32, device=self.dev)
+        have, results = {}, {}
+        own = lambda t, r: t[r * n:(r + 1) * n]
+
+        def on_transfer(tensor, src, dst, item, slot):
+            if tensor == SAP_T_Q:
+                self.stage_q[dst, slot].copy_(own(q, src))
+            elif tensor == SAP_T_KV:
+                self.stage_kv[dst, slot, 0].copy_(own(k, src)); self.stage_kv[dst, slot, 1].copy_(own(v, src))
+            elif tensor == SAP_T_DO:                          # dO rows with their LSE and D
+                self.stage_do[dst, slot].copy_(own(dout, src))
+                self.stage_dol[dst, slot, 0].copy_(lse[:, src * n:(src + 1) * n]); self.stage_dol[dst, slot, 1].copy_(dsum(ws_own)[:, src * n:(src + 1) * n])
+            elif tensor == SAP_T_DQ:
+                self.stage_dq[dst, slot].copy_(results.pop((src, SAP_T_DQ, item)))
+            else:
+                self.stage_dkv[dst, slot].copy_(results.pop((src, SAP_T_DKV, item)))
+
+        def on_compute(r, item):
+            i, j = int(self.items[item, 0]), int(self.items[item, 1])
+            assert r in (i, j)
+            if i == r:
+                qs, dos, ws, lse_g = own(q, r), own(dout, r), ws_own, lse
+            else:       # helper: Q, dO (with LSE, D) of chunk i arrived; contributions to dQ go to scratch rows of chunk i
+                assert have.pop((r, SAP_T_Q, item), False) and have.pop((r, SAP_T_DO, item), False), f"rank {r}: q / do of item {item} missing"
+                qs, dos, ws = self.comp_q[r], self.comp_do[r], ws_help
+                lse_g = self.part_l
+                lse_g[:, i * n:(i + 1) * n].copy_(self.comp_dol[r, 0]); dsum(ws)[:, i * n:(i + 1) * n].copy_(self.comp_dol[r, 1])
+                dqacc(ws)[i * n:(i + 1) * n].zero_()
+            if j == r:
+                ks, vs = own(k, r), own(v, r)
+            else:
+                assert have.pop((r, SAP_T_KV, item), False), f"rank {r}: K/V of item {item} missing"
+                ks, vs = self.comp_kv[r, 0], self.comp_kv[r, 1]
+            view = lambda t, c: ShardView(t.contiguous(), c * n, N)
+            api.sap_attn_bwd_items(view(dos, i), view(qs, i), view(ks, j), view(vs, j), lse_g, cu_seqlens_dev, self.plan, item, item + 1,
+                                   view(self.scratch_dkv[0], j), view(self.scratch_dkv[1], j), ws, softmax_scale=self.scale)
+            it = self.items[item]
+            kb, ke = int(it[8]) - j * n, int(it[9]) - j * n      # the item's key rows inside chunk j (other rows of touched tiles: zero)
+            if j == r:
+                api.sap_axpy(dkv_tot[0, j * n + kb:j * n + ke], self.scratch_dkv[0, kb:ke], 1.0)
+                api.sap_axpy(dkv_tot[1, j * n + kb:j * n + ke], self.scratch_dkv[1, kb:ke], 1.0)
+            else:
+                c = torch.zeros_like(self.scratch_dkv); c[:, kb:ke] = self.scratch_dkv[:, kb:ke]
+                results[(r, SAP_T_DKV, item)] = c
+            if i != r:
+                results[(r, SAP_T_DQ, item)] = dqacc(ws)[i * n:(i + 1) * n].clone()
+
+        def on_copy(r, tensor, peer, item, slot):
+            if tensor == SAP_T_Q:
+                self.comp_q[r].copy_(self.stage_q[r, slot]); have[(r, tensor, item)] = True
+            elif tensor == SAP_T_KV:
+                self.comp_kv[r].copy_(self.stage_kv[r, slot]); have[(r, tensor, item)] = True
+            elif tensor == SAP_T_DO:
+                self.comp_do[r].copy_(self.stage_do[r, slot]); self.comp_dol[r].copy_(self.stage_dol[r, slot]); have[(r, tensor, item)] = True
+            elif tensor == SAP_T_DQ:                          # a received dq contribution is added into the owner's accumulator
+                api.sap_axpy(dqacc(ws_own)[r * n:(r + 1) * n], self.stage_dq[r, slot], 1.0)
+            else:
+                api.sap_axpy(dkv_tot[0, r * n:(r + 1) * n], self.stage_dkv[r, slot, 0], 1.0)
+                api.sap_axpy(dkv_tot[1, r * n:(r + 1) * n], self.stage_dkv[r, slot, 1], 1.0)
+
+        self._walk(self.bwd_codes, on_transfer, on_compute, on_copy)
+        assert not have and not results, "every transferred tensor was consumed"
+        dq = torch.empty_like(q)
+        for r in range(P):
+            api.sap_attn_bwd_end(self.plan, r, r + 1, dq, Hkv, ws_own, softmax_scale=self.scale)
+        dk, dv = torch.empty_like(k), torch.empty_like(v)
+        api.sap_axpy(dk, dkv_tot[0], 1.0, accumulate=False); api.sap_axpy(dv, dkv_tot[1], 1.0, accumulate=False)
+        return dq, dk, dv

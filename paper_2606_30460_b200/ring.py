@@ -50,6 +50,9 @@ def sap_ring_fwd(kv_shard, plan: Plan, rank: int, partial_fn: Callable, merge_fn
 
     P = plan.n_chunks
     assert dist.get_world_size(group) == P, "one rank per sequence chunk"
+    # `rank` and the plan's chunk indices are ranks INSIDE `group` (HSAP runs the SAP ring over an inter-group
+    # sub-communicator); P2POp wants global ranks
+    glob = (lambda r: r) if group is None else (lambda r: dist.get_global_rank(group, r))
     items = plan.items
     co = plan.chunk_offsets
     my_items = {int(items[x, 1]): x for x in range(int(co[rank]), int(co[rank + 1]))}   # kv_chunk -> item index
@@ -59,10 +62,10 @@ def sap_ring_fwd(kv_shard, plan: Plan, rank: int, partial_fn: Callable, merge_fn
         dst, src = step_peers(plan, rank, step)
         ops, buf = [], None
         if dst is not None:
-            ops.append(dist.P2POp(dist.isend, kv_shard, dst, group))
+            ops.append(dist.P2POp(dist.isend, kv_shard, glob(dst), group))
         if src is not None:
             buf = torch.empty_like(kv_shard)
-            ops.append(dist.P2POp(dist.irecv, buf, src, group))
+            ops.append(dist.P2POp(dist.irecv, buf, glob(src), group))
         return (dist.batch_isend_irecv(ops) if ops else []), buf
 
     nxt = post(1) if P > 1 else ([], None)
@@ -80,29 +83,31 @@ def sap_ring_fwd(kv_shard, plan: Plan, rank: int, partial_fn: Callable, merge_fn
 
 
 def cuda_fns(q_shard, cu_seqlens_dev, plan: Plan, rank: int, softmax_scale: Optional[float] = None):
-    """(partial_fn, merge_fn) on the C-ABI kernels.  The kernels address tokens globally, so the rank keeps
-    full-length Q / K / V buffers of which only its own rows and the shard in flight are filled."""
+    """(partial_fn, merge_fn) on the C-ABI kernels.  The kernels address tokens globally; the shards are handed over as
+    executor.ShardView (base pointer moved back by the shard's first row) and the forward `computing` entry
+    sap_attn_fwd_items touches only the Q tiles of the item, so a rank holds its own Q rows, the K/V shard in flight
+    and one partial result: O(N/P) memory and work per item (only the per-row LSE buffer, 4 bytes per row and head,
+    is full length: the library's [Hq, N] layout)."""
     import torch
     from . import api
+    from .executor import ShardView
 
     n, Hq, d = q_shard.shape
     N = plan.n_tokens
     dev = q_shard.device
     lo, hi = rank * n, (rank + 1) * n
-    qg = torch.zeros((N, Hq, d), dtype=q_shard.dtype, device=dev)
-    qg[lo:hi] = q_shard
-    kg = vg = None
+    qg = ShardView(q_shard.contiguous(), lo, N)
+    lse_full = torch.empty((Hq, N), dtype=torch.float32, device=dev)
 
     def partial_fn(item, k_shard, v_shard):
-        nonlocal kg, vg
-        if kg is None:
-            kg = torch.zeros((N,) + tuple(k_shard.shape[1:]), dtype=k_shard.dtype, device=dev)
-            vg = torch.zeros_like(kg)
         j = int(plan.items[item, 1])
-        kg[j * n:(j + 1) * n] = k_shard
-        vg[j * n:(j + 1) * n] = v_shard
-        o, lse = api.sap_attn_fwd_partial(qg, kg, vg, cu_seqlens_dev, plan, item, item + 1, softmax_scale=softmax_scale)
-        return o[lo:hi].contiguous(), lse[:, lo:hi].contiguous()
+        Hkv = k_shard.shape[1]
+        o = torch.zeros((n, Hq, d), dtype=torch.float32, device=dev)   # Q tiles the item does not touch: the (0, -inf) identity
+        lse_full[:, lo:hi] = float("-inf")
+        api.sap_attn_fwd_items(qg, ShardView(k_shard.contiguous(), j * n, N), ShardView(v_shard.contiguous(), j * n, N),
+                               cu_seqlens_dev, plan, item, item + 1, ShardView(o, lo, N), lse_full, Hq, Hkv, d,
+                               softmax_scale=softmax_scale)
+        return o, lse_full[:, lo:hi].contiguous()
 
     def merge_fn(o_a, lse_a, o_b, lse_b):
         return api.sap_lse_merge(o_a, lse_a, o_b, lse_b)

@@ -30,9 +30,17 @@ def _inputs():
     return q, k, v
 
 
-def _worker(rank, world, port, out_q):
+def _worker(rank, world, port, out_q, sub=None):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     dist.init_process_group("gloo", rank=rank, world_size=world)
+    group = None
+    if sub is not None:           # the SAP ring runs over a strict subgroup whose ranks are not the global ranks
+        group = dist.new_group(sub)
+        if rank not in sub:
+            dist.barrier()        # stay until the ring is done: the members' connections run through this process group
+            dist.destroy_process_group()
+            return
+        rank, world = dist.get_group_rank(group, rank), len(sub)
     try:
         import paper_2606_30460_b200 as sap
         from paper_2606_30460_b200 import ring
@@ -62,10 +70,12 @@ def _worker(rank, world, port, out_q):
             return oracle.lse_merge(oa, la, ob, lb)
 
         kv = torch.stack([k[lo:hi], v[lo:hi]]).contiguous()
-        o, l = ring.sap_ring_fwd(kv, plan, rank, partial_fn, merge_fn)
+        o, l = ring.sap_ring_fwd(kv, plan, rank, partial_fn, merge_fn, group=group)
         o_ref, l_ref = oracle.attn_fwd(q.numpy(), k.numpy(), v.numpy(), cu, scale, rows=list(range(lo, hi)))
         want = sorted(int(plan.items[x, 1]) for x in range(int(plan.chunk_offsets[rank]), int(plan.chunk_offsets[rank + 1])))
         out_q.put((rank, float(np.abs(o - o_ref).max()), float(np.abs(l - l_ref).max()), sorted(received), want))
+        if sub is not None:
+            dist.barrier()
     finally:
         dist.destroy_process_group()
 
@@ -85,6 +95,23 @@ def test_ring_forward_matches_unchunked(world):
     for rank, eo, el, got, want in res:
         assert eo < 1e-12 and el < 1e-12, (rank, eo, el)
         assert got == want                      # exactly the shards the plan names: skipped pairs move no data
+
+
+def test_ring_over_a_subgroup_with_non_identity_ranks():
+    # world of 3, the ring over global ranks {0, 2}: group rank 1 is global rank 2 (HSAP's inter-group communicator)
+    ctx = mp.get_context("spawn")
+    out_q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 3, port, out_q, [2, 0])) for r in range(3)]
+    for p in procs:
+        p.start()
+    res = sorted(out_q.get(timeout=180) for _ in range(2))
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    assert [r[0] for r in res] == [0, 1]
+    for rank, eo, el, got, want in res:
+        assert eo < 1e-12 and el < 1e-12 and got == want
 
 
 def test_schedule_skips_what_the_plan_skips():
