@@ -6,8 +6,12 @@
 A step = one pass of the whole hot path (plan already compiled ahead): sap_attn_fwd
 (a2-a4) + sap_attn_bwd (a5-a7) over one seeded synthetic packed sequence of BASELINE.json configs[2]
 (128K tokens, log-normal documents, 16 chunks, 32/8 heads, d=128) — the configuration the metric is
-quoted on.  One JSON line on stdout (rank 0).  Multi-GPU: one process per GPU, independent sequences
-per rank (data-parallel units, no collective on the data path), weak scaling.
+quoted on.  One JSON line on stdout (rank 0).  Multi-GPU: one process per GPU (`--gpus N` without a torchrun
+environment starts the N ranks itself), no collective on the data path, two splits:
+  --shard seqs  (default) independent packed sequences per rank, seed = rank: weak scaling;
+  --shard heads one sequence, its kv-heads (with their q-heads) split over the ranks (heads are independent,
+                PAPER.md:65): zero exchange, strong scaling.
+`--dry-run` runs the host side only (planner, sharding, aggregation over gloo): no GPU needed.
 
 `--impl reference` times the fp64 CPU oracle (oracle/), as it stands, on a bounded sample.
 """
@@ -81,6 +85,9 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+ORACLE_SAMPLE_TOKENS = 2048   # the ONE sample both arms time the oracle on (about 6 s on 16 host threads)
+
+
 def cpu_sample_workload(n_tokens: int):
     """Bounded sample of configs[2] for the oracle: its leading documents, cut at n_tokens, all heads."""
     from paper_2606_30460_b200.workloads import custom_workload, make_workload
@@ -94,43 +101,39 @@ def cpu_sample_workload(n_tokens: int):
     return custom_workload(lens, 1, w3.n_q_heads, w3.n_kv_heads, w3.head_dim, name=f"cfg3_prefix_{n_tokens}")
 
 
-def time_oracle(n_tokens: int):
-    """fwd + dQ + dK/dV of the oracle on the sample; returns (seconds, useful flops, threads, description)."""
+def time_oracle(w, what: str):
+    """fwd + dQ + dK/dV of the oracle, as it stands, on workload w; returns (seconds, useful flops, threads, description)."""
     from oracle import oracle
     from paper_2606_30460_b200.workloads import make_qkv
-    w = cpu_sample_workload(n_tokens)
     q, k, v, do = (t.float().numpy() for t in make_qkv(w, device="cpu"))
     t0 = time.perf_counter()
     oracle.attn_fwd(q, k, v, w.cu_seqlens, w.softmax_scale)
     oracle.attn_bwd_dq(q, k, v, do, w.cu_seqlens, w.softmax_scale)
     oracle.attn_bwd_dkv(q, k, v, do, w.cu_seqlens, w.softmax_scale)
     dt = time.perf_counter() - t0
-    desc = (f"first {n_tokens} tokens of configs[2] (docs {list(w.doc_lens)}), {w.n_q_heads}/{w.n_kv_heads} heads, "
-            f"d={w.head_dim}: oracle fwd + dQ + dK/dV, every element")
+    desc = (f"{what} (docs {list(w.doc_lens)}), {w.n_q_heads}/{w.n_kv_heads} heads, d={w.head_dim}: oracle fwd + dQ + dK/dV, "
+            f"every element")
     return dt, w.flops_fwd + w.flops_bwd, oracle.num_threads(), desc
 
 
-def time_oracle_bounded(target_s: float):
-    """Calibrate on 1024 tokens (cost grows as n^2), then time a sample sized for about target_s seconds."""
-    dt, fl, th, desc = time_oracle(1024)
-    n = int(1024 * (target_s / max(dt, 1e-3)) ** 0.5) // 256 * 256
-    n = max(1024, min(n, 8192))
-    if n == 1024:
-        return dt, fl, th, desc
-    return time_oracle(n)
+def time_oracle_sample():
+    return time_oracle(cpu_sample_workload(ORACLE_SAMPLE_TOKENS), f"first {ORACLE_SAMPLE_TOKENS} tokens of configs[2]")
+
+
+def time_oracle_cfg1():
+    from paper_2606_30460_b200.workloads import make_workload
+    return time_oracle(make_workload(1), "configs[0] in full")
 
 
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    dt1 = time_oracle(512)[0]                         # calibrate: ~4 s of oracle work per step
-    n_tokens = max(512, min(int(512 * (4.0 / max(dt1, 1e-3)) ** 0.5) // 128 * 128, 4096))
     for _ in range(args.warmup):
-        time_oracle(256)
+        time_oracle(cpu_sample_workload(256), "warm-up")
     tot_t, tot_f, threads, desc = 0.0, 0, 0, ""
     for _ in range(args.steps):
-        dt, fl, threads, desc = time_oracle(n_tokens)
+        dt, fl, threads, desc = time_oracle_sample()       # every step = the same fixed sample the GPU arm's cpu_baseline uses
         tot_t += dt; tot_f += fl
     val = tot_f / tot_t / 1e12
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
@@ -141,6 +144,63 @@ def run_reference(args):
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+def kernel_source_sha256():
+    """Hash of every source file that goes into libsap_b200.so: the key of profiles/traffic.json."""
+    import hashlib
+    root = os.path.join(ROOT, "paper_2606_30460_b200", "csrc")
+    h = hashlib.sha256()
+    for f in sorted(os.listdir(root)):
+        h.update(f.encode()); h.update(open(os.path.join(root, f), "rb").read())
+    return h.hexdigest()
+
+
+def recorded_traffic(cfg: int, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on BASELINE.json configs[cfg-1], from the
+    committed ncu summary profiles/traffic.json - only if that capture was taken on this very kernel source."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(path):
+        return None, None
+    rec = json.load(open(path))
+    if rec.get("kernel_source_sha256") != kernel_source_sha256():
+        return None, "profiles/traffic.json was captured on another kernel source (hash differs): not reported"
+    val = rec.get("bytes_per_launch", {}).get(f"cfg{cfg}", {}).get(kernel)
+    return val, (rec.get("source") if val is not None else None)
+
+
+def spawn_ranks(args):
+    """`--gpus N` outside torchrun: start the N ranks (one process per GPU) under torch.distributed.run."""
+    import socket
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
+def run_dry(args):
+    """Host side only (no GPU): sharding, planner and the aggregation collectives over gloo."""
+    import torch.distributed as dist
+    from paper_2606_30460_b200 import shard
+    import paper_2606_30460_b200 as sap
+    rank, world, _ = shard.rank_world()
+    if world > 1:
+        dist.init_process_group("gloo")
+    w, heads = shard.rank_share(args.config, rank, world, args.shard)
+    plan = sap.sap_plan(w.cu_seqlens, w.n_chunks)
+    share = len(heads) / w.n_kv_heads
+    ms_max, flops_all = shard.aggregate(1.0 + rank, float(w.flops_fwd + w.flops_bwd) * share)
+    if rank == 0:
+        print(json.dumps({"dry_run": True, "metric": METRIC, "n_gpus": world, "shard": args.shard,
+                          "scaling": "strong" if args.shard == "heads" else "weak", "plan_items": plan.n_items,
+                          "kv_heads_of_rank0": list(heads), "whole_job_tflop_per_step": flops_all / 1e12,
+                          "max_over_ranks_check": ms_max == float(world),
+                          "config": {"workload": w.name, "n_tokens": w.n_tokens}}), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
 
 
 def run_ours(args):
@@ -158,13 +218,20 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    # each rank gets its own packed sequence (seed = rank): data-parallel units, no exchange
-    w = shard.rank_workload(args.config, rank)
+    # --shard seqs: each rank gets its own packed sequence (seed = rank): data-parallel units, no exchange;
+    # --shard heads: one sequence, rank r keeps kv-heads `heads` and their q-heads (heads are independent)
+    w, heads = shard.rank_share(args.config, rank, world, args.shard)
     q, k, v, do = make_qkv(w, device=dev)
+    g = w.n_q_heads // w.n_kv_heads
+    if len(heads) != w.n_kv_heads:
+        qsel = [hk * g + i for hk in heads for i in range(g)]
+        q, do = q[:, qsel].contiguous(), do[:, qsel].contiguous()
+        k, v = k[:, list(heads)].contiguous(), v[:, list(heads)].contiguous()
+    share = len(heads) / w.n_kv_heads
     plan = sap.sap_plan(w.cu_seqlens, w.n_chunks)
     plan.upload()
     cu = plan.cu_seqlens_dev(dev)
-    N, Hq, Hkv, d = w.n_tokens, w.n_q_heads, w.n_kv_heads, w.head_dim
+    N, Hq, Hkv, d = w.n_tokens, q.shape[1], k.shape[1], w.head_dim
     out = torch.empty_like(q); lse = torch.empty((Hq, N), dtype=torch.float32, device=dev)
     dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(v)
     ws = torch.empty(sap.sap_workspace_bytes(plan, Hq, Hkv, d, sap.SAP_PASS_BWD), dtype=torch.uint8, device=dev)
@@ -207,20 +274,28 @@ def run_ours(args):
     launches = sap.sap_launch_count() - launches0
     sync_all()
     clocks = sampler.stop() if rank == 0 else None
-    ms_max, flops_all = shard.aggregate(ms, float(w.flops_fwd + w.flops_bwd), dev)   # MAX time, SUM work
+    ms_max, flops_all = shard.aggregate(ms, float(w.flops_fwd + w.flops_bwd) * share, dev)   # MAX time, SUM work
     value = flops_all / (ms_max * 1e-3) / 1e12
 
     # ---- per-kernel times (separate passes; CUDA events on the launching stream), rank 0 reports
     kn = max(3, min(args.steps, 10))
     t_fwd = timed(fwd, kn)
     per = {}
-    stage_list = (("bwd_pre", 1), ("bwd_dkv", 2), ("bwd_dq", 4)) if args.bwd == "split" else \
-                 (("bwd_pre", 1), ("bwd_fused", 8), ("bwd_post", 16))
-    for name, mask in stage_list:
-        sap.sap_debug_set_bwd_stages(mask)
-        bwd(); torch.cuda.synchronize()
-        per[name] = timed(bwd, kn)
-    sap.sap_debug_set_bwd_stages(bwd_mask)
+    if args.bwd == "split":
+        for name, mask in (("bwd_pre", 1), ("bwd_dkv", 2), ("bwd_dq", 4)):
+            sap.sap_debug_set_bwd_stages(mask)
+            bwd(); torch.cuda.synchronize()
+            per[name] = timed(bwd, kn)
+        sap.sap_debug_set_bwd_stages(bwd_mask)
+    else:   # the three phases of sap_attn_bwd through their own entry points (the per-rank calls over all chunks)
+        P = w.n_chunks
+        phases = {"bwd_pre": lambda: sap.sap_attn_bwd_begin(do, out, plan, 0, P, Hkv, ws),
+                  "bwd_fused": lambda: sap.sap_attn_bwd_chunks(do, q, k, v, lse, cu, plan, 0, P, dk, dv, ws, softmax_scale=w.softmax_scale),
+                  "bwd_post": lambda: sap.sap_attn_bwd_end(plan, 0, P, dq, Hkv, ws, softmax_scale=w.softmax_scale)}
+        for name, fn in phases.items():
+            fn(); torch.cuda.synchronize()
+            per[name] = timed(fn, kn)
+    main_kernel = "sap_bwd_pair_kernel" if d == 128 else "sap_bwd_fused_kernel"
 
     # ---- end to end: host (pinned) buffers in, results back to host, copies inside the timed region
     if args.profile_only:
@@ -229,12 +304,12 @@ def run_ours(args):
         if rank == 0:
             bwd_ms = sum(per.values())
             print(json.dumps({"profile_only": True, "workload": w.name, "n_tokens": N, "n_docs": len(w.doc_lens),
-                              "useful_pairs": w.pairs, "plan_items": plan.n_items, "cu_seqlens_sha256": w.sha256(),
+                              "useful_pairs": w.pairs, "plan_items": plan.n_items, "cu_seqlens_sha256": w.sha256(), "shard": args.shard, "n_gpus": world,
                               "bwd": args.bwd, "ms_per_step": ms_max, "value": value,
                               "frac_of_measured_burst_peak": value / world / load_peaks()["bf16_burst"],
                               "tokens_per_s": N * world / (ms_max * 1e-3), "fwd_ms": t_fwd,
-                              "fwd_tflops": w.flops_fwd / (t_fwd * 1e-3) / 1e12, "bwd_ms": bwd_ms,
-                              "bwd_tflops": w.flops_bwd / (bwd_ms * 1e-3) / 1e12, **per, "clocks": clocks}))
+                              "fwd_tflops": w.flops_fwd * share / (t_fwd * 1e-3) / 1e12, "bwd_ms": bwd_ms,
+                              "bwd_tflops": w.flops_bwd * share / (bwd_ms * 1e-3) / 1e12, **per, "clocks": clocks}))
         return
     hq, hk, hv, hdo = (x.cpu().pin_memory() for x in (q, k, v, do))
     r_out, r_lse = torch.empty_like(hq).pin_memory(), torch.empty((Hq, N), dtype=torch.float32).pin_memory()
@@ -296,7 +371,7 @@ def run_ours(args):
         # algorithmic FLOPs per launch: 2*d flops per visible (row, key) pair per
         # q-head per GEMM; fwd = 2 GEMMs, dK/dV kernel = 4 of the backward's 5 (S, dP, dV, dK), dQ kernel = 1 (dQ;
         # its S/dP recompute is overhead, not algorithmic work)
-        gemm = 2.0 * d * Hq * pairs
+        gemm = 2.0 * d * Hq * pairs       # Hq = this rank's q-heads
         kernels = {
             "sap_fwd_kernel": {"ms": t_fwd, "algorithmic_tflop": 2 * gemm / 1e12},
             "sap_bwd_pre_kernel": {"ms": per["bwd_pre"], "algorithmic_gbytes": (2 * N * Hq * d * 2 + N * Hq * 4) / 1e9},
@@ -306,8 +381,8 @@ def run_ours(args):
             kernels["sap_bwd_dq_kernel"] = {"ms": per["bwd_dq"], "algorithmic_tflop": 1 * gemm / 1e12,
                                             "executed_tflop": 3 * gemm / 1e12}
         else:
-            # fused main kernel: all 5 GEMMs of the backward; its time includes zeroing the fp32 dQ accumulator
-            kernels["sap_bwd_fused_kernel"] = {"ms": per["bwd_fused"], "algorithmic_tflop": 5 * gemm / 1e12}
+            # main kernel: all 5 GEMMs of the backward (the D pre-pass line includes zeroing the fp32 dQ accumulator)
+            kernels[main_kernel] = {"ms": per["bwd_fused"], "algorithmic_tflop": 5 * gemm / 1e12}
             kernels["sap_bwd_post_kernel"] = {"ms": per["bwd_post"], "algorithmic_gbytes": N * Hq * d * 6 / 1e9}
         for kk, vv in kernels.items():
             if "algorithmic_tflop" in vv:
@@ -317,32 +392,36 @@ def run_ours(args):
                 vv["gbs"] = vv["algorithmic_gbytes"] / (vv["ms"] * 1e-3)
                 vv["frac_of_hbm"] = vv["gbs"] / peaks["hbm"]
         dom = max((kk for kk in kernels if "tflops" in kernels[kk]), key=lambda kk: kernels[kk]["ms"])
-        # DRAM bytes per launch of the dominant kernel from the one `ncu --set full` capture of this workload
-        # (profiles/r1c_ncu.md: dram__bytes_read.sum + dram__bytes_write.sum); no capture for other configurations
-        traffic = 13.172744e9 + 7.687649e9 if (dom == "sap_bwd_fused_kernel" and args.config == 3 and rank == 0) else None
+        # DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` summary, if it was taken
+        # on this kernel source and this configuration (null otherwise)
+        traffic, traffic_src = recorded_traffic(args.config, dom) if (world == 1 and args.shard == "seqs") else (None, None)
         roofline = {"kernel": dom, "bound": "tensor", "achieved": kernels[dom]["tflops"],
                     "peak": peaks["bf16_sustained"], "unit": "TFLOP/s",
                     "frac": kernels[dom]["tflops"] / peaks["bf16_sustained"], "traffic": traffic,
                     "peak_source": peaks["source"] + ", sustained bf16 (kernel timed inside a long step)",
                     "ms_per_launch": kernels[dom]["ms"],
-                    "traffic_source": "profiles/r1c_ncu.md (ncu --set full, one launch)" if traffic else None}
-        cdt, cfl, cthreads, cdesc = time_oracle_bounded(15.0)
+                    "traffic_source": traffic_src}
+        cdt, cfl, cthreads, cdesc = time_oracle_sample()
+        c1dt, c1fl, _, c1desc = time_oracle_cfg1()
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak",
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_max, "higher_is_better": True,
+            "scaling": "strong" if args.shard == "heads" else "weak",
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": (f"BASELINE.json configs[{args.config - 1}]: {w.name}" if args.config <= 5 else
                                     f"paper Table 2 shape (context, not a BASELINE config): {w.name}"), "n_tokens": N,
                        "n_chunks": w.n_chunks, "n_docs": len(w.doc_lens), "n_q_heads": Hq, "n_kv_heads": Hkv,
                        "head_dim": d, "cu_seqlens_sha256": w.sha256(), "useful_pairs": pairs,
                        "plan_items": plan.n_items, "l2": "inputs exceed L2 (Q alone is %.0f MiB)" % (q.numel() * 2 / 2**20),
-                       "per_rank": "independent sequence per rank (seed = rank)", "bwd": args.bwd},
+                       "per_rank": ("independent sequence per rank (seed = rank)" if args.shard == "seqs" else
+                                    f"one sequence, {Hkv} of its {w.n_kv_heads} kv-heads (and their q-heads) per rank, no exchange"),
+                       "shard": args.shard, "bwd": args.bwd},
             "tokens_per_s": N * world / (ms_max * 1e-3),
             "frac_of_bf16_peak": {"measured_burst": value / world / peaks["bf16_burst"],
                                   "measured_sustained": value / world / peaks["bf16_sustained"],
                                   "datasheet_2250": value / world / 2250.0, "source": peaks["source"]},
-            "fwd": {"ms": t_fwd, "tflops": w.flops_fwd / (t_fwd * 1e-3) / 1e12},
-            "bwd": {"ms": sum(per.values()), "tflops": w.flops_bwd / (sum(per.values()) * 1e-3) / 1e12},
+            "fwd": {"ms": t_fwd, "tflops": w.flops_fwd * share / (t_fwd * 1e-3) / 1e12},
+            "bwd": {"ms": sum(per.values()), "tflops": w.flops_bwd * share / (sum(per.values()) * 1e-3) / 1e12},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": ms_e2e_max, "steps": e_steps,
@@ -351,7 +430,8 @@ def run_ours(args):
             "roofline": roofline,
             "kernels": kernels,
             "cpu_baseline": {"value": cfl / cdt / 1e12, "unit": UNIT, "cores": cthreads, "kind": "oracle",
-                             "sample": cdesc, "seconds": cdt},
+                             "sample": cdesc, "seconds": cdt,
+                             "cfg1_full": {"value": c1fl / c1dt / 1e12, "unit": UNIT, "seconds": c1dt, "sample": c1desc}},
             "paper_context": "HSAP Table 2 (PAPER.md:158-164): SAP attention fwd+bwd 128K/SP16 = 3333.1 ms on A100s, "
                              "multi-GPU, communication included; not comparable, context only",
         }
@@ -372,11 +452,18 @@ def main():
                     help="forward kernel: two q-heads per CTA (default when Hq/Hkv is even) or one (diagnostic)")
     ap.add_argument("--bwd", default="fused", choices=["fused", "split"],
                     help="backward form: fused 5-GEMM kernel (default) or the split dK/dV + dQ kernels (diagnostic)")
+    ap.add_argument("--shard", default="seqs", choices=["seqs", "heads"],
+                    help="multi-GPU split: independent sequences per rank (weak scaling) or the kv-heads of one sequence (strong)")
+    ap.add_argument("--dry-run", action="store_true", help="host side only (planner, sharding, aggregation over gloo); no GPU")
     ap.add_argument("--profile-only", action="store_true",
                     help="stop after the device-timed region and the per-kernel passes (for ncu runs)")
     args = ap.parse_args()
+    if args.gpus > 1 and "RANK" not in os.environ and args.impl == "ours":
+        spawn_ranks(args)              # one process per GPU; this process only waits for them
     if args.impl == "reference":
         run_reference(args)
+    elif args.dry_run:
+        run_dry(args)
     else:
         run_ours(args)
 

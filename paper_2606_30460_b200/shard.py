@@ -26,6 +26,21 @@ def rank_workload(cfg: int, rank: int) -> Workload:
     return make_workload(cfg, seed=rank)
 
 
+def rank_share(cfg: int, rank: int, world: int, how: str = "seqs"):
+    """(workload, kv-heads) of rank `rank`.  how = "seqs": its own sequence (seed = rank), all heads (weak scaling);
+    how = "heads": THE sequence (seed 0) and an equal contiguous share of its kv-heads - heads are independent
+    (multi-head attention "as H independent single head attention"; IntraSP shards them, :65), so the
+    ranks exchange nothing (strong scaling)."""
+    if how == "seqs":
+        w = rank_workload(cfg, rank)
+        return w, tuple(range(w.n_kv_heads))
+    w = rank_workload(cfg, 0)
+    if w.n_kv_heads % world != 0:
+        raise ValueError(f"--shard heads needs n_kv_heads ({w.n_kv_heads}) divisible by the number of ranks ({world})")
+    per = w.n_kv_heads // world
+    return w, tuple(range(rank * per, (rank + 1) * per))
+
+
 def _dist():
     import torch.distributed as dist
     return dist if dist.is_available() and dist.is_initialized() else None
