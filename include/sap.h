@@ -264,6 +264,17 @@ const char* sap_strerror(int status);
 int sap_last_cuda_error(void);      /* the cudaError_t / CUresult of the last SAP_ERR_CUDA on this thread */
 /* Number of kernels the library has launched in this process (all streams); for launch accounting. */
 int64_t sap_launch_count(void);
+/* Diagnostic (host only, no GPU): the tile program the kernels walk, as flat int32 records - tiles [n][4] = (row0, rows,
+ * seg_begin, seg_end) of each stationary tile, segs [n][8] = (t_begin, t_end, q_lo, q_hi, kv_lo, kv_hi, item, 0) of each
+ * run of streamed tiles: element (row t, key s) of a (tile, segment) is computed iff t (Q-stationary) or s
+ * (K/V-stationary) lies in the tile, the other index in [t_begin, t_end), q_lo <= t < q_hi, kv_lo <= s < kv_hi, both in
+ * one document and s <= t.  kind: 0 forward (Q-stationary), 1 / 2 backward K/V-stationary with 128- / 256-key tiles;
+ * 3 / 4 items [a, b) Q-stationary (all tiles / touched tiles: sap_attn_fwd_partial / sap_attn_fwd_items); 5 q-chunks
+ * [a, b) (sap_attn_fwd_chunks); 6 / 7 kv-chunks [a, b) with 128- / 256-key tiles (sap_attn_bwd_chunks); 8 / 9 items
+ * [a, b) K/V-stationary (sap_attn_bwd_items).  Returns the number of tiles (call with null buffers to size), *n_segs
+ * the number of segments; < 0 on error.  Buffers are filled only when large enough. */
+int32_t sap_debug_tile_program(const sap_plan_t* plan, int32_t kind, int32_t a, int32_t b, int32_t* tiles, int32_t tiles_cap,
+                               int32_t* segs, int32_t segs_cap, int32_t* n_segs);
 /* Diagnostic: which forward kernel sap_attn_fwd / sap_attn_fwd_partial launch.  0 (default): the pair kernel (two
  * q-heads of one GQA group per CTA, sharing the K/V tiles) whenever Hq/Hkv is even, the one-head kernel otherwise;
  * 1: always the one-head kernel.  Process-wide; returns the previous value. */

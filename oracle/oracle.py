@@ -4,10 +4,12 @@ TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and
 bench.py's cpu_baseline / --impl reference leg may import this.  It imports nothing
 from paper_2606_30460_b200 (the CUDA path) and shares no code with it.
 
-Parity status: every float function and plan() are pinned (tests/test_oracle_*.py); schedule() (compile Steps 2-3)
-and codegen() (jitted code generation) are PARTIALLY PINNED - validity, closed forms, bounds, send/recv pairing and
-the replay test are pinned; the choice among valid schedules and the stage offsets are a reading (R-5; the
-paper's Fig. 3 is missing).
+Parity status: every float function and plan() are pinned (tests/test_oracle_*.py).  For the compile side of the
+NEXT rows the oracle no longer mirrors the library: min_makespan() is the exhaustive definition of the best possible
+makespan (pinned by closed forms) and check_codes() is a legality checker of instruction lists written from Table 1 and
+PAPER.md:100-102,:120-124 (pinned by hand-made legal and illegal lists) - neither generates a schedule or a code list.
+schedule() remains as the step-by-step restatement of the reading DESIGN.md R-5 (the paper's Fig. 3 is missing): it
+pins that the library implements that reading, the reading itself is scored against min_makespan().
 
 Arrays are numpy; Q/K/V/dO are float32 arrays holding bf16-exact values
 (`tensor.float().numpy()`); every result is float64.
@@ -207,9 +209,9 @@ def schedule(cu_seqlens, n_chunks: int, policy: int = 1):
     most one item per stage: it runs its items back to back in order of (regional stage, i, j), stage = position
     in that list (:118; shards travel point to point, so any order is legal); before that, Step 3a moves items off the busiest rank while
     that lowers its load ("striving to balance the computation load across all SAP ranks globally", :118).
-    PARITY: pinned by validity (every item once, rank in {i, j}, one item per rank and stage), by the closed form
-    for one document (floor(P/2) + 1 stages, loads within 1) and by makespan bounds; the choice among valid
-    schedules is this reading's, not the paper's (figure missing) - "partially pinned".
+    PARITY: this function restates the reading R-5; what pins the READING is min_makespan(): on every tiny layout
+    (P <= 6, <= 3 documents) the makespan of this schedule is within one block of the exhaustive optimum, and equal
+    to it for a single document (tests/test_schedule.py).
     """
     pl = plan(cu_seqlens, n_chunks)
     cu = [int(x) for x in cu_seqlens]
@@ -266,79 +268,135 @@ def schedule(cu_seqlens, n_chunks: int, policy: int = 1):
     return slots, (int(slots[:, 1].max()) + 1 if len(items) else 0)
 
 
+def min_makespan(cu_seqlens, n_chunks: int, limit: int = 1 << 22):
+    """The smallest makespan, in block units, ANY assignment of plan items to ranks can reach (Steps
+    2-3 decide "which rank computes each block" and "the stage index"; one block per rank and stage): every DIAG item
+    runs on its own rank, every FULL item (i, j) on rank i (K/V_j travels) or on rank j (Q_i travels, the partial
+    travels back); a rank runs its items back to back, so the makespan is the largest number of items on one rank.
+    Exhaustive over the 2^(#FULL) assignments - the definition, no heuristic; tiny inputs only."""
+    pl = plan(cu_seqlens, n_chunks)
+    P = int(n_chunks)
+    load0 = [0] * P
+    full = []
+    for row in pl.items:
+        i, j, kind = int(row[0]), int(row[1]), int(row[4])
+        if kind == DIAG:
+            load0[i] += 1
+        else:
+            full.append((i, j))
+    if (1 << len(full)) > limit:
+        raise ValueError("too many FULL items for the exhaustive search")
+    best = None
+    for mask in range(1 << len(full)):
+        load = list(load0)
+        for b, (i, j) in enumerate(full):
+            load[j if (mask >> b) & 1 else i] += 1
+        m = max(load)
+        best = m if best is None or m < best else best
+    return best if best is not None else 0
+
+
 OP_SEND, OP_RECV, OP_COMPUTING, OP_COPY = 0, 1, 2, 3
-T_Q, T_KV, T_O = 0, 1, 2
+T_Q, T_KV, T_O, T_DO, T_DQ, T_DKV = 0, 1, 2, 3, 4, 5
 
 
-def codegen(cu_seqlens, n_chunks: int, slots, rank: int):
-    """Jitted code generation for the forward pass (Table 1 :85-98), written out rule by rule.
-    Codes are (stage, opcode, tensor, peer, item).  For every plan item (i, j) with slot (R, st):
-      R runs `computing item` at stage st;
-      if i != j and R == i: kv travels j -> i at stage st-1 (send on j, recv + copy on i);
-      if i != j and R == j: q travels i -> j at stage st-1 (send on i, recv + copy on j) and the partial result o
-                            travels j -> i at stage st+1 (send on j, recv + copy-and-rescale on i).
-    Order inside a stage: SEND/RECV by (opcode, tensor, peer, item), then COMPUTING, then COPY by (tensor, peer, item).
-    PARITY: the transport rules above are the paper's (who needs which tensor follows from where the block runs);
-    the stage offsets (-1 / +1) and the order inside a stage are this build's reading - partially pinned: pinned by
-    the executor test (every rank's replay reproduces the unchunked attention) and by send/recv pairing."""
+def check_codes(cu_seqlens, n_chunks: int, slots, code_lists, backward: bool = False):
+    """Legality of the instruction lists of ALL ranks (code_lists[r] = int array [n, 5] of (stage, opcode, tensor, peer,
+    item)) for a schedule `slots` - a checker, not a generator: any list that passes can be executed, whatever stage
+    offsets or in-stage order its author chose.  Returns a list of violations (empty = legal).  Rules, each from the
+    paper's description of the execute side (Table 1):
+
+      R1  a rank walks its list stage by stage; inside a stage the SEND / RECV codes come first (one batched
+          isend/irecv, in flight while the block is computed, :122-124), then COMPUTING, then COPY (:102).
+      R2  every plan item is computed exactly once, by the rank and at the stage its slot names, and a rank computes at
+          most one item per stage (:116-118).
+      R3  operands are in the compute buffer before COMPUTING: an item (i, j) computed on rank R != i needs q of chunk i
+          (and, backward, do) - RECV from i and COPY at a stage EARLIER than the computing stage; R != j needs kv of
+          chunk j the same way.  A rank never receives a tensor it owns or does not need ("trim redundant
+          communication", :106).
+      R4  every SEND has its RECV with the same (stage, tensor, item) on the peer and vice versa ("send/recv pairs
+          aligned", :124), sent by the rank that owns / produced the tensor; every RECV has its COPY in the same or a
+          later stage on the same rank.
+      R5  what a rank computes for another is returned AFTER it exists: forward, R != i sends the partial o to i at a
+          stage LATER than the computing stage; backward, R != i returns dq to i and R != j returns dkv to j.  Nothing
+          else travels.
+    """
     pl = plan(cu_seqlens, n_chunks)
-    out = []
-    for x, row in enumerate(pl.items):
-        i, j = int(row[0]), int(row[1])
-        R, st = int(slots[x][0]), int(slots[x][1])
-        if R == rank:
-            out.append((st, OP_COMPUTING, -1, -1, x))
-        if i == j:
-            continue
-        if R == i:
-            if rank == j:
-                out.append((st - 1, OP_SEND, T_KV, i, x))
-            if rank == i:
-                out += [(st - 1, OP_RECV, T_KV, j, x), (st - 1, OP_COPY, T_KV, j, x)]
-        else:
-            if rank == i:
-                out += [(st - 1, OP_SEND, T_Q, j, x), (st + 1, OP_RECV, T_O, j, x), (st + 1, OP_COPY, T_O, j, x)]
-            if rank == j:
-                out += [(st - 1, OP_RECV, T_Q, i, x), (st - 1, OP_COPY, T_Q, i, x), (st + 1, OP_SEND, T_O, i, x)]
+    P = int(n_chunks)
+    items = [(int(r[0]), int(r[1])) for r in pl.items]
+    bad = []
+    sends, recvs, copies, computes = {}, {}, {}, {}
     phase = {OP_SEND: 0, OP_RECV: 0, OP_COMPUTING: 1, OP_COPY: 2}
-    out.sort(key=lambda c: (c[0], phase[c[1]], c[1] if phase[c[1]] == 0 else 0, c[2], c[3], c[4]))
-    return np.array(out, dtype=np.int32).reshape(-1, 5)
-
-
-T_DO, T_DQ, T_DKV = 3, 4, 5
-
-
-def codegen_bwd(cu_seqlens, n_chunks: int, slots, rank: int):
-    """Backward instruction list of `rank` (tensors do / dq / dkv of Table 1), rule by rule:
-      R == i: kv travels j -> i at stage st-1, the dK/dV contribution (dkv) travels i -> j at stage st+1;
-      R == j: q and do (with LSE, D) travel i -> j at stage st-1, the dQ contribution (dq) travels j -> i at st+1.
-    Same format and order as codegen().  Partially pinned, as codegen()."""
-    pl = plan(cu_seqlens, n_chunks)
-    out = []
-
-    def transfer(stage, tensor, src, dst, x):
-        if rank == src:
-            out.append((stage, OP_SEND, tensor, dst, x))
-        if rank == dst:
-            out.extend([(stage, OP_RECV, tensor, src, x), (stage, OP_COPY, tensor, src, x)])
-
-    for x, row in enumerate(pl.items):
-        i, j = int(row[0]), int(row[1])
+    for r in range(P):
+        last = None
+        per_stage = {}
+        for st, op, tensor, peer, item in (tuple(int(v) for v in c) for c in code_lists[r]):
+            key = (st, phase.get(op, 9))
+            if last is not None and key < last:
+                bad.append(f"R1 rank {r}: code (stage {st}, opcode {op}) is out of order")
+            last = key
+            if not 0 <= item < len(items):
+                bad.append(f"rank {r}: item {item} does not exist"); continue
+            if op == OP_COMPUTING:
+                if item in computes:
+                    bad.append(f"R2 item {item} computed twice")
+                computes[item] = (r, st)
+                per_stage[st] = per_stage.get(st, 0) + 1
+                if per_stage[st] > 1:
+                    bad.append(f"R2 rank {r} computes two items at stage {st}")
+            elif op == OP_SEND:
+                if (tensor, r, peer, item) in sends: bad.append(f"R4 duplicate SEND {(tensor, r, peer, item)}")
+                sends[(tensor, r, peer, item)] = st
+            elif op == OP_RECV:
+                if (tensor, peer, r, item) in recvs: bad.append(f"R4 duplicate RECV {(tensor, peer, r, item)}")
+                recvs[(tensor, peer, r, item)] = st
+            elif op == OP_COPY:
+                copies[(tensor, peer, r, item)] = st
+            else:
+                bad.append(f"rank {r}: unknown opcode {op}")
+    for x, (i, j) in enumerate(items):
         R, st = int(slots[x][0]), int(slots[x][1])
-        if R == rank:
-            out.append((st, OP_COMPUTING, -1, -1, x))
-        if i == j:
-            continue
-        if R == i:
-            transfer(st - 1, T_KV, j, i, x)
-            transfer(st + 1, T_DKV, i, j, x)
-        else:
-            transfer(st - 1, T_Q, i, j, x)
-            transfer(st - 1, T_DO, i, j, x)
-            transfer(st + 1, T_DQ, j, i, x)
-    phase = {OP_SEND: 0, OP_RECV: 0, OP_COMPUTING: 1, OP_COPY: 2}
-    out.sort(key=lambda c: (c[0], phase[c[1]], c[1] if phase[c[1]] == 0 else 0, c[2], c[3], c[4]))
-    return np.array(out, dtype=np.int32).reshape(-1, 5)
+        if computes.get(x) != (R, st):
+            bad.append(f"R2 item {x} computed at {computes.get(x)}, its slot says {(R, st)}")
+    if set(sends) != set(recvs):
+        bad.append(f"R4 unpaired SEND / RECV: {sorted(set(sends) ^ set(recvs))[:4]}")
+    for key in set(sends) & set(recvs):
+        if sends[key] != recvs[key]:
+            bad.append(f"R4 SEND at stage {sends[key]} but RECV at stage {recvs[key]} for {key}")
+        if key not in copies or copies[key] < recvs[key]:
+            bad.append(f"R4 RECV {key} has no COPY in the same or a later stage")
+    if set(copies) - set(recvs):
+        bad.append(f"R4 COPY without RECV: {sorted(set(copies) - set(recvs))[:4]}")
+    need = set()          # every transfer the schedule requires, as (tensor, src, dst, item) with its stage constraint
+    for x, (i, j) in enumerate(items):
+        R, st = int(slots[x][0]), int(slots[x][1])
+        ops_in = []
+        if R != i:
+            ops_in += [(T_Q, i)] + ([(T_DO, i)] if backward else [])
+        if R != j:
+            ops_in += [(T_KV, j)]
+        for tensor, src in ops_in:                                    # R3
+            key = (tensor, src, R, x)
+            need.add(key)
+            if key not in copies:
+                bad.append(f"R3 item {x} on rank {R}: tensor {tensor} of chunk {src} never arrives")
+            elif copies[key] >= st:
+                bad.append(f"R3 item {x} computed at stage {st} but tensor {tensor} is copied at stage {copies[key]}")
+        outs = []
+        if R != i:
+            outs.append((T_DQ if backward else T_O, i))
+        if backward and R != j:
+            outs.append((T_DKV, j))
+        for tensor, dst in outs:                                      # R5
+            key = (tensor, R, dst, x)
+            need.add(key)
+            if key not in sends:
+                bad.append(f"R5 item {x}: result tensor {tensor} is never returned to rank {dst}")
+            elif sends[key] <= st:
+                bad.append(f"R5 item {x} computed at stage {st} but its result is sent at stage {sends[key]}")
+    if set(sends) - need:
+        bad.append(f"R3/R5 transfers nobody needs: {sorted(set(sends) - need)[:4]}")
+    return bad
 
 
 def attn_bwd_item(q, k, v, dout, lse, dsum, cu_seqlens, scale: float, q_begin: int, q_end: int, kv_begin: int,

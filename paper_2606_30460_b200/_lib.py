@@ -61,6 +61,8 @@ SIGNATURES = {
     "sap_strerror": (ctypes.c_char_p, [ctypes.c_int]),
     "sap_last_cuda_error": (ctypes.c_int, []),
     "sap_launch_count": (ctypes.c_int64, []),
+    "sap_debug_tile_program": (ctypes.c_int32, [vp, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, vp, ctypes.c_int32, vp,
+                                                ctypes.c_int32, c_i32p]),
     "sap_debug_set_bwd_stages": (ctypes.c_int, [ctypes.c_int]),
     "sap_debug_set_fwd_form": (ctypes.c_int, [ctypes.c_int]),
     "sap_debug_set_bwd_form": (ctypes.c_int, [ctypes.c_int]),

@@ -127,6 +127,18 @@ class Plan:
         fn(self._h, sl.ctypes.data_as(ctypes.c_void_p), int(rank), codes.ctypes.data_as(ctypes.c_void_p), n)
         return codes[:n]
 
+    def tile_program(self, kind: int, a: int = 0, b: int = 0):
+        """Diagnostic: (tiles int32 [n,4], segs int32 [m,8]) of the compiled tile program `kind` (sap_debug_tile_program)."""
+        L = _lib.lib()
+        ns = ctypes.c_int32(0)
+        nt = int(L.sap_debug_tile_program(self._h, int(kind), int(a), int(b), None, 0, None, 0, ctypes.byref(ns)))
+        if nt < 0:
+            raise SapError(-nt, "sap_debug_tile_program")
+        tiles = np.zeros((max(nt, 1), 4), dtype=np.int32); segs = np.zeros((max(ns.value, 1), 8), dtype=np.int32)
+        L.sap_debug_tile_program(self._h, int(kind), int(a), int(b), tiles.ctypes.data_as(ctypes.c_void_p), nt,
+                                 segs.ctypes.data_as(ctypes.c_void_p), ns.value, ctypes.byref(ns))
+        return tiles[:nt], segs[:ns.value]
+
     def upload(self):
         _check(_lib.lib().sap_plan_upload(self._h), "sap_plan_upload")
 

@@ -343,6 +343,33 @@ int32_t sap_plan_codegen_bwd(const sap_plan_t* p, const sap_slot_t* slots, int32
   return emit_codes(out, codes, cap);
 }
 
+int32_t sap_debug_tile_program(const sap_plan_t* p, int32_t kind, int32_t a, int32_t b, int32_t* tiles, int32_t tiles_cap,
+                               int32_t* segs, int32_t segs_cap, int32_t* n_segs) {
+  if (!p || !n_segs || tiles_cap < 0 || segs_cap < 0) return -SAP_ERR_INVALID_ARG;
+  TileProgram built;
+  const TileProgram* prog = &built;
+  const int32_t n_items = (int32_t)p->items.size();
+  auto items_ok = [&]() { return a >= 0 && b >= a && b <= n_items; };
+  auto chunks_ok = [&]() { return a >= 0 && b >= a && b <= p->n_chunks; };
+  switch (kind) {
+    case 0: prog = &p->fwd; break;
+    case 1: prog = &p->kv; break;
+    case 2: prog = &p->kv2; break;
+    case 3: if (!items_ok()) return -SAP_ERR_INVALID_ARG; build_q_program(*p, a, b, built, false); break;
+    case 4: if (!items_ok()) return -SAP_ERR_INVALID_ARG; build_q_program(*p, a, b, built, true); break;
+    case 5: if (!chunks_ok()) return -SAP_ERR_INVALID_ARG; build_q_program(*p, p->chunk_offsets[a], p->chunk_offsets[b], built, true); break;
+    case 6: case 7: if (!chunks_ok()) return -SAP_ERR_INVALID_ARG; build_kv_program(*p, built, a, b, kind == 7 ? 2 * kTile : kTile); break;
+    case 8: case 9: if (!items_ok()) return -SAP_ERR_INVALID_ARG; build_kv_program(*p, built, 0, -1, kind == 9 ? 2 * kTile : kTile, a, b, true); break;
+    default: return -SAP_ERR_INVALID_ARG;
+  }
+  static_assert(sizeof(TileDesc) == 4 * sizeof(int32_t) && sizeof(SegDesc) == 8 * sizeof(int32_t), "flat int32 records");
+  const int32_t nt = (int32_t)prog->tiles.size(), ns = (int32_t)prog->segs.size();
+  *n_segs = ns;
+  if (tiles && nt <= tiles_cap) std::memcpy(tiles, prog->tiles.data(), sizeof(TileDesc) * nt);
+  if (segs && ns <= segs_cap) std::memcpy(segs, prog->segs.data(), sizeof(SegDesc) * ns);
+  return nt;
+}
+
 const char* sap_strerror(int status) {
   switch (status) {
     case SAP_OK: return "ok";

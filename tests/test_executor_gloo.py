@@ -1,5 +1,6 @@
 """compile (sap_plan_schedule + sap_plan_codegen) -> execute (executor.sap_execute_fwd) with real
-ranks on CPU (gloo).  Code lists are bit-exact against the oracle's rule-by-rule version and pair up across ranks;
+ranks on CPU (gloo).  Code lists pass the oracle's legality checker (oracle.check_codes: operands present before
+`computing`, transfers paired, every partial returned, nothing redundant - a checker, not a second generator);
 replaying them - with the ORACLE as the compute callable, the schedule is what is under test - reproduces the
 unchunked attention on every rank, for the plain ring and for the balanced schedule (helpers compute on the K/V
 rank, Q travels there, the partial result travels back)."""
@@ -26,15 +27,15 @@ def cu_of(docs):
 @pytest.mark.parametrize("name", list(LAYOUTS))
 @pytest.mark.parametrize("P", [2, 4, 8])
 @pytest.mark.parametrize("policy", [0, 1])
-def test_codes_match_oracle_and_pair_up(name, P, policy):
+def test_codes_are_legal_and_pair_up(name, P, policy):
     cu = cu_of(LAYOUTS[name])
     plan = sap.sap_plan(cu, P)
     slots, n_stages = plan.schedule(policy)
     sends, recvs, computed = set(), set(), []
+    lists = [plan.codegen(slots, r) for r in range(P)]
+    assert oracle.check_codes(cu, P, slots, lists) == [], (name, P, policy)
     for r in range(P):
-        codes = plan.codegen(slots, r)
-        ref = oracle.codegen(cu, P, slots, r)
-        assert codes.tobytes() == ref.tobytes(), (name, P, policy, r)
+        codes = lists[r]
         assert (np.diff(codes[:, 0]) >= 0).all() and codes[:, 0].min() >= -1 and codes[:, 0].max() <= n_stages
         for st, op, tensor, peer, item in codes.tolist():
             if op == sap.SAP_OP_SEND:
@@ -117,15 +118,15 @@ def test_replaying_the_codes_reproduces_attention(docs, world, policy):
 @pytest.mark.parametrize("name", list(LAYOUTS))
 @pytest.mark.parametrize("P", [2, 4, 8])
 @pytest.mark.parametrize("policy", [0, 1])
-def test_bwd_codes_match_oracle_and_pair_up(name, P, policy):
+def test_bwd_codes_are_legal_and_pair_up(name, P, policy):
     cu = cu_of(LAYOUTS[name])
     plan = sap.sap_plan(cu, P)
     slots, n_stages = plan.schedule(policy)
     sends, recvs, computed = set(), set(), []
+    lists = [plan.codegen(slots, r, backward=True) for r in range(P)]
+    assert oracle.check_codes(cu, P, slots, lists, backward=True) == [], (name, P, policy)
     for r in range(P):
-        codes = plan.codegen(slots, r, backward=True)
-        ref = oracle.codegen_bwd(cu, P, slots, r)
-        assert codes.tobytes() == ref.tobytes(), (name, P, policy, r)
+        codes = lists[r]
         for st, op, tensor, peer, item in codes.tolist():
             if op == sap.SAP_OP_SEND:
                 sends.add((st, tensor, r, peer, item))
