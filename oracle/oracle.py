@@ -26,6 +26,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "sap_oracle.cpp")
 _LIB = os.path.join(_HERE, "libsap_oracle.so")
+_LIB_OVERRIDE = os.environ.get("SAP_ORACLE_LIB")   # an instrumented build (ASan / UBSan run)
 
 SKIP, FULL, DIAG = 0, 1, 2
 ITEM_FIELDS = ("q_chunk", "kv_chunk", "doc_lo", "doc_hi", "mask_kind", "step",
@@ -47,7 +48,7 @@ _lib = None
 def lib():
     global _lib
     if _lib is None:
-        _lib = ctypes.CDLL(build())
+        _lib = ctypes.CDLL(_LIB_OVERRIDE or build())
         _lib.sap_oracle_num_threads.restype = ctypes.c_int
     return _lib
 

@@ -365,8 +365,8 @@ int32_t sap_debug_tile_program(const sap_plan_t* p, int32_t kind, int32_t a, int
   static_assert(sizeof(TileDesc) == 4 * sizeof(int32_t) && sizeof(SegDesc) == 8 * sizeof(int32_t), "flat int32 records");
   const int32_t nt = (int32_t)prog->tiles.size(), ns = (int32_t)prog->segs.size();
   *n_segs = ns;
-  if (tiles && nt <= tiles_cap) std::memcpy(tiles, prog->tiles.data(), sizeof(TileDesc) * nt);
-  if (segs && ns <= segs_cap) std::memcpy(segs, prog->segs.data(), sizeof(SegDesc) * ns);
+  if (tiles && nt > 0 && nt <= tiles_cap) std::memcpy(tiles, prog->tiles.data(), sizeof(TileDesc) * nt);
+  if (segs && ns > 0 && ns <= segs_cap) std::memcpy(segs, prog->segs.data(), sizeof(SegDesc) * ns);
   return nt;
 }
 
