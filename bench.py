@@ -146,6 +146,44 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+PAPER_TABLE2_SAP_MS = {8192: 7.9, 16384: 11.1, 32768: 73.0, 65536: 1912.3, 131072: 3333.1}   # PAPER.md:158-164 (A100s, multi-GPU)
+
+
+def table2_context(dev, steps: int = 5):
+    """fwd+bwd time of one attention on the paper's Table 2 shape (16 heads MHA, d = 128, chunks =
+    SP size; the paper's length mix is not stated, the recipe of configs[2] stands in), beside the paper's own SAP
+    figure for that column - other hardware, transport included there: context, not a comparison."""
+    import torch
+    import paper_2606_30460_b200 as sap
+    from paper_2606_30460_b200.workloads import make_qkv, make_table2_workload
+    res = {}
+    for L in (8192, 32768, 131072):
+        w = make_table2_workload(L)
+        q, k, v, do = make_qkv(w, device=dev)
+        plan = sap.sap_plan(w.cu_seqlens, w.n_chunks); plan.upload()
+        cu = plan.cu_seqlens_dev(dev)
+        out = torch.empty_like(q); lse = torch.empty((w.n_q_heads, L), dtype=torch.float32, device=dev)
+        dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(v)
+        ws = torch.empty(sap.sap_workspace_bytes(plan, w.n_q_heads, w.n_kv_heads, w.head_dim, sap.SAP_PASS_BWD), dtype=torch.uint8, device=dev)
+
+        def step():
+            sap.sap_attn_fwd(q, k, v, cu, plan, out, lse, softmax_scale=w.softmax_scale)
+            sap.sap_attn_bwd(do, q, k, v, out, lse, cu, plan, softmax_scale=w.softmax_scale, dq=dq, dk=dk, dv=dv, workspace=ws)
+
+        for _ in range(3):
+            step()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); e0.record()
+        for _ in range(steps):
+            step()
+        e1.record(); torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        res[f"{L // 1024}K/SP{w.n_chunks}"] = {"ms_fwd_bwd": ms, "tflops": (w.flops_fwd + w.flops_bwd) / (ms * 1e-3) / 1e12,
+                                               "n_docs": len(w.doc_lens), "paper_sap_ms_a100_multi_gpu": PAPER_TABLE2_SAP_MS[L]}
+        del q, k, v, do, out, lse, dq, dk, dv, ws
+    return res
+
+
 def kernel_source_sha256():
     """Hash of every source file that goes into libsap_b200.so: the key of profiles/traffic.json."""
     import hashlib
@@ -401,6 +439,7 @@ def run_ours(args):
                     "peak_source": peaks["source"] + ", sustained bf16 (kernel timed inside a long step)",
                     "ms_per_launch": kernels[dom]["ms"],
                     "traffic_source": traffic_src}
+        t2 = table2_context(dev) if (world == 1 and args.config == 3) else None
         cdt, cfl, cthreads, cdesc = time_oracle_sample()
         c1dt, c1fl, _, c1desc = time_oracle_cfg1()
         line = {
@@ -432,6 +471,7 @@ def run_ours(args):
             "cpu_baseline": {"value": cfl / cdt / 1e12, "unit": UNIT, "cores": cthreads, "kind": "oracle",
                              "sample": cdesc, "seconds": cdt,
                              "cfg1_full": {"value": c1fl / c1dt / 1e12, "unit": UNIT, "seconds": c1dt, "sample": c1desc}},
+            "table2_context": t2,
             "paper_context": "HSAP Table 2 (PAPER.md:158-164): SAP attention fwd+bwd 128K/SP16 = 3333.1 ms on A100s, "
                              "multi-GPU, communication included; not comparable, context only",
         }

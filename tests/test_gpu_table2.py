@@ -1,0 +1,72 @@
+"""the shape of the paper's own attention micro-benchmark (Table 2: 16 heads
+MHA, "hidden_size" = head_dim 128) at 64K tokens / SP 16, in the launch configuration bench.py times - sampled rows
+(out, LSE, dQ) and key columns (dK, dV) against the fp64 oracle, plus the sparse-dO pass over every key column.
+MHA means an odd group size (1): the forward runs the one-head kernel, the backward the CTA-pair kernel with one q-head
+per K/V tile.  The paper's document-length mix is not stated; the log-normal recipe of configs[2] stands in."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_30460_b200 as sap
+from oracle import oracle
+from paper_2606_30460_b200.workloads import make_qkv, make_table2_workload
+from parity import check_close, check_lse, col_scale, row_scale, to_np
+
+pytestmark = pytest.mark.gpu
+
+
+def test_table2_shape_64k_sp16_sampled_against_oracle():
+    w = make_table2_workload(65536)
+    assert (w.n_q_heads, w.n_kv_heads, w.head_dim, w.n_chunks) == (16, 16, 128, 16)
+    N = w.n_tokens
+    heads = [0, 7, 15]
+    rng = np.random.default_rng(64)
+    q, k, v, do = make_qkv(w, device="cuda")
+    plan = sap.sap_plan(w.cu_seqlens, w.n_chunks)
+    ref_plan = oracle.plan(w.cu_seqlens, w.n_chunks)
+    assert plan.items.tobytes() == ref_plan.items.tobytes() and plan.kind_map.tobytes() == ref_plan.kind_map.tobytes()
+    cu = plan.cu_seqlens_dev("cuda")
+    n0 = sap.sap_launch_count()
+    out, lse = sap.sap_attn_fwd(q, k, v, cu, plan, softmax_scale=w.softmax_scale)
+    dq = torch.full_like(q, float("nan")); dk = torch.full_like(k, float("nan")); dv = torch.full_like(v, float("nan"))
+    sap.sap_attn_bwd(do, q, k, v, out, lse, cu, plan, softmax_scale=w.softmax_scale, dq=dq, dk=dk, dv=dv)
+    torch.cuda.synchronize()
+    assert sap.sap_launch_count() - n0 == 4
+    for name, t in (("out", out), ("lse", lse), ("dq", dq), ("dk", dk), ("dv", dv)):
+        assert bool(torch.isfinite(t).all()), f"{name}: non-finite values"
+    args = (to_np(q[:, heads]), to_np(k[:, heads]), to_np(v[:, heads]))
+    dos = to_np(do[:, heads])
+    cuv, n = w.cu_seqlens, N // w.n_chunks
+    rows = set(int(t) for t in rng.integers(0, N, size=192))
+    for e in range(len(w.doc_lens)):
+        if w.doc_lens[e] > 0:
+            rows.update((cuv[e], cuv[e + 1] - 1))
+    for i in range(1, w.n_chunks):
+        rows.update((i * n - 1, i * n))
+    rows = np.array(sorted(rows), dtype=np.int64)
+    rt = torch.from_numpy(rows).cuda()
+    nat = row_scale(cuv, rows)
+    o_ref, l_ref = oracle.attn_fwd(*args, cuv, w.softmax_scale, rows=rows)
+    check_close(to_np(out[rt][:, heads]), o_ref, "table2 64K out", nat)
+    check_lse(to_np(lse[heads][:, rt]).T, l_ref, "table2 64K lse")
+    check_close(to_np(dq[rt][:, heads]), oracle.attn_bwd_dq(*args, dos, cuv, w.softmax_scale, rows=rows), "table2 64K dq", nat)
+    docs = sorted(range(len(w.doc_lens)), key=lambda e: -w.doc_lens[e])
+    cols = set()
+    for e in docs[:3]:
+        cols.update(range(max(cuv[e], cuv[e + 1] - 64), cuv[e + 1]))
+    for e in [e for e in docs if 0 < w.doc_lens[e] <= 1024][:4]:
+        cols.update(range(cuv[e], cuv[e + 1]))
+    cols = np.array(sorted(cols), dtype=np.int64)
+    ct = torch.from_numpy(cols).cuda()
+    dk_ref, dv_ref = oracle.attn_bwd_dkv(*args, dos, cuv, w.softmax_scale, cols=cols)
+    check_close(to_np(dk[ct][:, heads]), dk_ref, "table2 64K dk", col_scale(cuv, cols))
+    check_close(to_np(dv[ct][:, heads]), dv_ref, "table2 64K dv", col_scale(cuv, cols))
+    # sparse dO: every key column against a seeded set of live rows
+    live = np.unique(rng.integers(0, N, size=256))
+    lt = torch.from_numpy(live).cuda()
+    do_sp = torch.zeros_like(do); do_sp[lt] = do[lt]
+    dq2, dk2, dv2 = sap.sap_attn_bwd(do_sp, q, k, v, out, lse, cu, plan, softmax_scale=w.softmax_scale)
+    torch.cuda.synchronize()
+    dk_ref2, dv_ref2 = oracle.attn_bwd_dkv(*args, to_np(do_sp[:, heads]), cuv, w.softmax_scale)
+    check_close(to_np(dk2[:, heads]), dk_ref2, "table2 64K dk, sparse dO, all columns")
+    check_close(to_np(dv2[:, heads]), dv_ref2, "table2 64K dv, sparse dO, all columns")
