@@ -21,9 +21,10 @@
 //   dQ^T is drained with red.global.add.f32 into dq_acc [N,Hq,d] (lane = d index: one 128-byte line per warp and row).
 //
 // TMEM (512 columns per CTA): [0,128) dK | [128,256) dV | two score buffers b at 256 + 128 b:
-//   [0,64) S^T fp32 -> per 16 q rows k: P^T bf16 at [16k, 16k+8), dS^T bf16 at [16k+8, 16k+16)
-//   [64,128) dP^T fp32; dQ^T of tile j lands at [64,96) of buffer (j+1)&1 (over dP^T of tile j+1, already read):
-//            lane = 64 (q / 32) + (d % 64), column = q % 32  (cta_group::2, M = 128 layout)
+//   [0,64)   S^T fp32, free again as soon as the compute warps have read it; dQ^T of tile j then lands at [0,32) of buffer
+//            (j+1)&1 (over S^T of tile j+1): lane = 64 (q / 32) + (d % 64), column = q % 32  (cta_group::2, M = 128 layout)
+//   [64,128) dP^T fp32 -> per 16 q rows k: P^T bf16 at [64+16k, 64+16k+8), dS^T bf16 at [64+16k+8, 64+16k+16)
+//            (the A operands of dV / dK: this region is the one with the long life, S^T(i+2) does not wait for it)
 // Shared memory per CTA (224 KB): K 32 | V 32 | K^T 32 ([256 keys x own 64 d]) | Q 3 x 16 | dO 3 x 16 | dS^T 2 x 16.
 //   A Q (dO) stage holds the four 32-row x 64-column boxes the CTA's B halves need, each at the same offset in both
 //   CTAs because one descriptor addresses both: rows of q half r (both d halves) for S^T (dP^T), columns of d half r
@@ -214,16 +215,17 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
       const uint64_t dQm0 = make_smem_desc(sQ + 2 * L::kQSlot, 2 * L::kQSlot, 1024);                // MN-major: d half r
       const uint64_t dDOm0 = make_smem_desc(sDO + 2 * L::kQSlot, 2 * L::kQSlot, 1024);
       const uint64_t dDS0 = make_smem_desc_sw(sDS, 4096, 512, kSwizzle64B);                         // dS^T: MN-major B, 32 q per CTA
-      mbar_poll(bar_kv_full, 0);
+      mbar_wait(bar_kv_full, 0);
       // Two issuing threads feed the one tensor pipe (it runs the MMAs in arrival order): this one S^T(i), dP^T(i); the
       // elected thread of warp 3 dQ^T(j), dV/dK(j).  Each waits only for its own inputs, so no cross-CTA hand-off of one
       // stream (200-600 cycles each) delays the other.  Every ordering between the streams is a barrier:
-      //   S^T(i)  after dV/dK(i-2) have read P^T / dS^T from these columns        (dvk_done, committed by warp 3)
-      //   dP^T(i) after dQ^T(i-3) was drained from these columns in both CTAs      (dq_empty)
+      //   S^T(i)  after S^T(i-2) was read and dQ^T(i-3) drained from these columns (dpr, dq_empty; both CTAs)
+      //   dP^T(i) after dV/dK(i-2) have read P^T / dS^T from these columns        (dvk_done, committed by warp 3)
       for (int i = 0; i < n_iters; ++i) {
         const int b = i & 1, st = i % kPairStages;
-        mbar_poll(bar_qs_full + 8 * st, (i / kPairStages) & 1);
-        if (i >= 2) mbar_poll(bar_dvk_done + 8 * b, ((i - 2) >> 1) & 1);
+        mbar_wait(bar_qs_full + 8 * st, (i / kPairStages) & 1);
+        if (i >= 2) mbar_wait(bar_dpr + 8 * b, ((i - 2) >> 1) & 1);              // S^T(i-2) has been read from these columns
+        if (i >= 3) mbar_wait(bar_dq_empty + 8 * (b ^ 1), ((i - 3) >> 1) & 1);   // ... and dQ^T(i-3), which followed it there, drained
         tc_fence_after();
         SAP_STAMP2(i, 18);
         const uint64_t dq = desc_add(dQs0, st * L::kQBytes), ddo = desc_add(dDOs0, st * L::kQBytes);
@@ -231,7 +233,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
         for (int k = 0; k < D / 16; ++k)
           umma2_ss(tBuf + 128 * b, desc_add(dK0, (k / 4) * L::kKVBox + (k % 4) * 32), desc_add(dq, (k / 4) * L::kQSlot + (k % 4) * 32), idesc_s, k > 0);
         SAP_STAMP2(i, 0);
-        if (i >= 3) { mbar_poll(bar_dq_empty + 8 * (b ^ 1), ((i - 3) >> 1) & 1); tc_fence_after(); }
+        if (i >= 2) { mbar_wait(bar_dvk_done + 8 * b, ((i - 2) >> 1) & 1); tc_fence_after(); }   // dV/dK(i-2) have read P^T, dS^T there
         SAP_STAMP2(i, 17);
 #pragma unroll
         for (int k = 0; k < D / 16; ++k)
@@ -260,29 +262,29 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
       const uint64_t dDS0 = make_smem_desc_sw(sDS, 4096, 512, kSwizzle64B);                         // dS^T: MN-major B, 32 q per CTA
       for (int j = 0; j <= n_iters; ++j) {
         if (j >= 1) {
-          const int q = j - 1, b = q & 1;   // dS^T buffer b; dQ^T goes to the dP^T columns of the other score buffer
-          mbar_poll(bar_ds_land + 8 * b, (q >> 1) & 1);   // this CTA's dS^T buffer is complete
-          mbar_poll(bar_ds_full + 8 * b, (q >> 1) & 1);   // ... and the peer's
+          const int q = j - 1, b = q & 1;   // dS^T buffer b; dQ^T goes to the S^T columns of the other score buffer
+          mbar_wait(bar_ds_land + 8 * b, (q >> 1) & 1);   // this CTA's dS^T buffer is complete
+          mbar_wait(bar_ds_full + 8 * b, (q >> 1) & 1);   // ... and the peer's
           fence_proxy_async_smem();
-          if (q + 1 < n_iters) mbar_poll(bar_dpr + 8 * (b ^ 1), ((q + 1) >> 1) & 1);               // dP^T(q+1) has been read
-          else if (q >= 2) mbar_poll(bar_dq_empty + 8 * b, ((q - 2) >> 1) & 1);                      // last tile: dQ^T(q-2) drained
+          if (q + 1 < n_iters) mbar_wait(bar_dpr + 8 * (b ^ 1), ((q + 1) >> 1) & 1);               // S^T(q+1) has been read
+          else if (q >= 2) mbar_wait(bar_dq_empty + 8 * b, ((q - 2) >> 1) & 1);                      // last tile: dQ^T(q-2) drained
           tc_fence_after();
           SAP_STAMP2(q, 12);
           const uint64_t dsb = desc_add(dDS0, b * L::kDSBytes);
 #pragma unroll
           for (int k = 0; k < kPairKeys / 16; ++k)  // 16 keys per MMA
-            umma2_ss(tBuf + 128 * (b ^ 1) + 64, desc_add(dKT0, k * 2048), desc_add(dsb, k * 1024), idesc_dq, k > 0);
+            umma2_ss(tBuf + 128 * (b ^ 1), desc_add(dKT0, k * 2048), desc_add(dsb, k * 1024), idesc_dq, k > 0);
           umma2_commit(bar_dq_full + 8 * b, 3);
           if (q == n_iters - 1) umma2_commit(bar_acc_full, 3);
           SAP_STAMP2(q, 4);
         }
         if (j < n_iters) {
           const int bj = j & 1, stj = j % kPairStages;
-          mbar_poll(bar_qm_full + 8 * stj, (j / kPairStages) & 1);
-          mbar_poll(bar_p_full + 8 * bj, (j >> 1) & 1);
+          mbar_wait(bar_qm_full + 8 * stj, (j / kPairStages) & 1);
+          mbar_wait(bar_p_full + 8 * bj, (j >> 1) & 1);
           tc_fence_after();
           SAP_STAMP2(j, 15);
-          const uint32_t tPT = tBuf + 128 * bj;
+          const uint32_t tPT = tBuf + 128 * bj + 64;
           const uint64_t dqm = desc_add(dQm0, stj * L::kQBytes), ddom = desc_add(dDOm0, stj * L::kQBytes);
 #pragma unroll
           for (int k = 0; k < kBwdN / 16; ++k)
@@ -319,7 +321,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
           tc_fence_after();
           if (warp == 4 + 4 * kFusedParts && lane == 0) SAP_STAMP2(j, 8);
           uint32_t v[kCols];
-          tmem_ld16(tBuf + 128 * (b ^ 1) + 64 + lane_base + kCols * dpart, v);
+          tmem_ld16(tBuf + 128 * (b ^ 1) + lane_base + kCols * dpart, v);
           tmem_wait_ld();
           tc_fence_before();
           __syncwarp();
@@ -391,7 +393,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
             if (warp == 4 && lane == 0 && pp == 0) SAP_STAMP2(i, 23);
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) { if (cta == 0) mbar_arrive(bar_dpr + 8 * b); else mbar_arrive_cluster_relaxed(lead_dpr + 8 * b); }   // these dP^T columns may take dQ^T(i-1)
+            if (lane == 0) { if (cta == 0) mbar_arrive(bar_dpr + 8 * b); else mbar_arrive_cluster_relaxed(lead_dpr + 8 * b); }   // S^T and dP^T of this part are in registers: the S^T columns may take dQ^T(i-1)
             if (lane == 0) { SAP_STAMP_MAX(i, 22); }
             if (need_mask) {  // boundary tiles only: masked scores become -inf, so P = 2^-inf = 0 and dS = 0
 #pragma unroll
@@ -417,7 +419,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
               pk[kFusedCols / 2 + q4 * 2 + 1] = dsk[pp][q4 * 2 + 1] = pack_bf16x2(ds[2], ds[3]);
             }
             if (warp == 4 && lane == 0 && pp == 0) SAP_STAMP2(i, 24);
-            tmem_st16(tST, pk);   // bf16 P^T and dS^T over the 16 S^T columns just read
+            tmem_st16(tDPT, pk);  // bf16 P^T and dS^T over the 16 dP^T columns just read
             tmem_wait_st();
             if (warp == 4 && lane == 0 && pp == 0) SAP_STAMP2(i, 25);
             tc_fence_before();
