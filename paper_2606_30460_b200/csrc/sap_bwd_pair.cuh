@@ -85,7 +85,8 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
                  bar_p_full = smem_u32(bars + 15) /*L*/, bar_acc_full = smem_u32(bars + 17) /*B*/,
                  bar_dq_full = smem_u32(bars + 18) /*B*/, bar_dq_empty = smem_u32(bars + 20) /*L*/,
                  bar_ds_full = smem_u32(bars + 22) /*L: relay from the peer*/, bar_ds_land = smem_u32(bars + 24) /*own CTA*/,
-                 bar_dpr = smem_u32(bars + 26) /*L*/, bar_dvk_done = smem_u32(bars + 34) /*leader: dV/dK(j) have read P^T, dS^T*/;
+                 bar_dpr = smem_u32(bars + 26) /*L*/, bar_dvk_done = smem_u32(bars + 34) /*leader: dV/dK(j) have read P^T, dS^T*/,
+                 bar_p_full2 = smem_u32(bars + 36) /*L: second column part of every compute warp*/;
 
   // logical warp id: service warps (0-3) are the physically last four (see sap_fwd.cuh)
   const int warp = ((threadIdx.x >> 5) + 4) % (kPairThreads / 32), lane = threadIdx.x & 31;
@@ -104,7 +105,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
       mbar_init(bar_stat_full + 8 * i, 32); mbar_init(bar_stat_empty + 8 * i, 2 * 4);
     }
     for (int i = 0; i < 2; ++i) {
-      mbar_init(bar_s_full + 8 * i, 1); mbar_init(bar_p_full + 8 * i, 2 * 4 * kFusedParts);
+      mbar_init(bar_s_full + 8 * i, 1); mbar_init(bar_p_full + 8 * i, 2 * 4 * 2); mbar_init(bar_p_full2 + 8 * i, 2 * 4 * 2);
       mbar_init(bar_dq_full + 8 * i, 1); mbar_init(bar_dq_empty + 8 * i, 2 * 4 * kFusedDrainGroups);
       mbar_init(bar_ds_full + 8 * i, 1); mbar_init(bar_ds_land + 8 * i, 4); mbar_init(bar_dpr + 8 * i, 2 * 4 * kFusedParts);
       mbar_init(bar_dvk_done + 8 * i, 1);
@@ -281,17 +282,21 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
         if (j < n_iters) {
           const int bj = j & 1, stj = j % kPairStages;
           mbar_wait(bar_qm_full + 8 * stj, (j / kPairStages) & 1);
-          mbar_wait(bar_p_full + 8 * bj, (j >> 1) & 1);
-          tc_fence_after();
           SAP_STAMP2(j, 15);
           const uint32_t tPT = tBuf + 128 * bj + 64;
           const uint64_t dqm = desc_add(dQm0, stj * L::kQBytes), ddom = desc_add(dDOm0, stj * L::kQBytes);
+          // k = 16 q rows = one column part; every compute warp finishes its first part (k even) well before its second
 #pragma unroll
-          for (int k = 0; k < kBwdN / 16; ++k)
-            umma2_ts(tDV, tPT + k * 16, desc_add(ddom, k * 2048), idesc_acc, (j > 0 || k > 0) ? 1u : 0u);
+          for (int pp = 0; pp < 2; ++pp) {
+            mbar_wait((pp ? bar_p_full2 : bar_p_full) + 8 * bj, (j >> 1) & 1);
+            tc_fence_after();
 #pragma unroll
-          for (int k = 0; k < kBwdN / 16; ++k)
-            umma2_ts(tDK, tPT + k * 16 + 8, desc_add(dqm, k * 2048), idesc_acc, (j > 0 || k > 0) ? 1u : 0u);
+            for (int k = pp; k < kBwdN / 16; k += 2)
+              umma2_ts(tDV, tPT + k * 16, desc_add(ddom, k * 2048), idesc_acc, (j > 0 || k > 0) ? 1u : 0u);
+#pragma unroll
+            for (int k = pp; k < kBwdN / 16; k += 2)
+              umma2_ts(tDK, tPT + k * 16 + 8, desc_add(dqm, k * 2048), idesc_acc, (j > 0 || k > 0) ? 1u : 0u);
+          }
           umma2_commit(bar_qm_empty + 8 * stj, 3);
           umma2_commit(bar_dvk_done + 8 * bj, 1);
           SAP_STAMP2(j, 3);
@@ -356,7 +361,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
     // 64-byte swizzle (chunk ^= bits 7-8 of the byte offset)
     const uint32_t prow = static_cast<uint32_t>(kTile * cta + r) * 64, psw = ((prow >> 7) & 3) << 4;
     const uint32_t ds_dst = mapa_cluster(sDS, static_cast<uint32_t>(qh));
-    const uint32_t lead_p_full = mapa_cluster(bar_p_full, 0), lead_dpr = mapa_cluster(bar_dpr, 0);
+    const uint32_t lead_p_full = mapa_cluster(bar_p_full, 0), lead_p_full2 = mapa_cluster(bar_p_full2, 0), lead_dpr = mapa_cluster(bar_dpr, 0);
     const uint32_t peer_ds_land = mapa_cluster(bar_ds_land, cta ^ 1);
     const bool ds_expect = quarter == 0;   // one of the 4 local-storing warps of a tile announces the peer's bytes
     uint8_t* const ds_local = (static_cast<uint32_t>(qh) == cta) ? smem + L::kOffDS : nullptr;  // own q half: plain stores
@@ -393,7 +398,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
             if (warp == 4 && lane == 0 && pp == 0) SAP_STAMP2(i, 23);
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) { if (cta == 0) mbar_arrive(bar_dpr + 8 * b); else mbar_arrive_cluster_relaxed(lead_dpr + 8 * b); }   // S^T and dP^T of this part are in registers: the S^T columns may take dQ^T(i-1)
+            if (lane == 0) mbar_arrive_cluster_relaxed(lead_dpr + 8 * b);   // S^T and dP^T of this part are in registers: the S^T columns may take dQ^T(i-1).  (Both CTAs arrive through the cluster window: no branch on the CTA rank)
             if (lane == 0) { SAP_STAMP_MAX(i, 22); }
             if (need_mask) {  // boundary tiles only: masked scores become -inf, so P = 2^-inf = 0 and dS = 0
 #pragma unroll
@@ -424,7 +429,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
             if (warp == 4 && lane == 0 && pp == 0) SAP_STAMP2(i, 25);
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) { if (cta == 0) mbar_arrive(bar_p_full + 8 * b); else mbar_arrive_cluster_relaxed(lead_p_full + 8 * b); }   // dV / dK of this tile may start
+            if (lane == 0) mbar_arrive_cluster_relaxed((pp ? lead_p_full2 : lead_p_full) + 8 * b);   // the dV / dK steps over these 16 q rows may start
             if (lane == 0) { SAP_STAMP_MAX(i, 20); SAP_STAMP_MIN(i, 21); }
           }
           if (i >= 2) mbar_wait(bar_dq_full + 8 * b, ((i >> 1) - 1) & 1);  // dQ^T of tile i-2 has read dS^T buffer b
