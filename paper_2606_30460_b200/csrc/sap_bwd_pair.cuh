@@ -86,7 +86,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
                  bar_dq_full = smem_u32(bars + 18) /*B*/, bar_dq_empty = smem_u32(bars + 20) /*L*/,
                  bar_ds_full = smem_u32(bars + 22) /*L: relay from the peer*/, bar_ds_land = smem_u32(bars + 24) /*own CTA*/,
                  bar_dpr = smem_u32(bars + 26) /*L*/, bar_dvk_done = smem_u32(bars + 34) /*leader: dV/dK(j) have read P^T, dS^T*/,
-                 bar_p_full2 = smem_u32(bars + 36) /*L: second column part of every compute warp*/;
+                 bar_p_full2 = smem_u32(bars + 36) /*L: second column part of every compute warp*/, bar_dpr2 = smem_u32(bars + 38) /*L: same for dpr*/;
 
   // logical warp id: service warps (0-3) are the physically last four (see sap_fwd.cuh)
   const int warp = ((threadIdx.x >> 5) + 4) % (kPairThreads / 32), lane = threadIdx.x & 31;
@@ -107,7 +107,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
     for (int i = 0; i < 2; ++i) {
       mbar_init(bar_s_full + 8 * i, 1); mbar_init(bar_p_full + 8 * i, 2 * 4 * 2); mbar_init(bar_p_full2 + 8 * i, 2 * 4 * 2);
       mbar_init(bar_dq_full + 8 * i, 1); mbar_init(bar_dq_empty + 8 * i, 2 * 4 * kFusedDrainGroups);
-      mbar_init(bar_ds_full + 8 * i, 1); mbar_init(bar_ds_land + 8 * i, 4); mbar_init(bar_dpr + 8 * i, 2 * 4 * kFusedParts);
+      mbar_init(bar_ds_full + 8 * i, 1); mbar_init(bar_ds_land + 8 * i, 4); mbar_init(bar_dpr + 8 * i, 2 * 4 * 2); mbar_init(bar_dpr2 + 8 * i, 2 * 4 * 2);
       mbar_init(bar_dvk_done + 8 * i, 1);
     }
     mbar_init(bar_acc_full, 1);
@@ -179,7 +179,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
       if (ph_prev >= 0) load_m(ph_prev, pt0, pst, pph);
     }
   } else if (warp == 2) {
-    // ------------------------------------------------------------------ per-row LSE (log2 domain) and D loader
+    // ------------------------------------------------------------------ per-row -LSE (log2 domain) and -D loader (negated: they are the addends of packed fma / add)
     int i = 0;
     for (int hq = 0; hq < g; ++hq) {
       const int h = hk * g + hq;
@@ -193,8 +193,8 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
 #pragma unroll
           for (int j = 0; j < 2; ++j) {
             const int t = t0 + lane + 32 * j;
-            a[j] = t < n_tokens ? __ldg(lse_h + t) * kLog2e : CUDART_INF_F;
-            b[j] = t < n_tokens ? __ldg(dsum_h + t) : 0.f;
+            a[j] = t < n_tokens ? -__ldg(lse_h + t) * kLog2e : -CUDART_INF_F;
+            b[j] = t < n_tokens ? -__ldg(dsum_h + t) : 0.f;
           }
           mbar_wait(bar_stat_empty + 8 * st, ((i / kPairStages) & 1) ^ 1);
 #pragma unroll
@@ -225,7 +225,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
       for (int i = 0; i < n_iters; ++i) {
         const int b = i & 1, st = i % kPairStages;
         mbar_wait(bar_qs_full + 8 * st, (i / kPairStages) & 1);
-        if (i >= 2) mbar_wait(bar_dpr + 8 * b, ((i - 2) >> 1) & 1);              // S^T(i-2) has been read from these columns
+        if (i >= 2) mbar_wait(bar_dpr2 + 8 * b, ((i - 2) >> 1) & 1);             // S^T(i-2) has been read from these columns (second parts last)
         if (i >= 3) mbar_wait(bar_dq_empty + 8 * (b ^ 1), ((i - 3) >> 1) & 1);   // ... and dQ^T(i-3), which followed it there, drained
         tc_fence_after();
         SAP_STAMP2(i, 18);
@@ -261,13 +261,18 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
       const uint64_t dQm0 = make_smem_desc(sQ + 2 * L::kQSlot, 2 * L::kQSlot, 1024);                // MN-major: d half r
       const uint64_t dDOm0 = make_smem_desc(sDO + 2 * L::kQSlot, 2 * L::kQSlot, 1024);
       const uint64_t dDS0 = make_smem_desc_sw(sDS, 4096, 512, kSwizzle64B);                         // dS^T: MN-major B, 32 q per CTA
+      // Per tile j: dQ^T of tile j-1, then the dV / dK steps of tile j, those over the first column parts (q rows [0,32))
+      // as soon as these are stored.  (dV / dK first halves ahead of dQ^T measured slower: 66.3 against 64.7 ms.)
       for (int j = 0; j <= n_iters; ++j) {
+        const int bj = j & 1, stj = j % kPairStages;
+        const uint32_t tPT = tBuf + 128 * bj + 64;
+        const uint64_t dqm = desc_add(dQm0, stj * L::kQBytes), ddom = desc_add(dDOm0, stj * L::kQBytes);
         if (j >= 1) {
-          const int q = j - 1, b = q & 1;   // dS^T buffer b; dQ^T goes to the S^T columns of the other score buffer
+          const int q = j - 1, b = q & 1;   // dS^T buffer b; dQ^T goes to columns [0,32) of the S^T region of the other score buffer
           mbar_wait(bar_ds_land + 8 * b, (q >> 1) & 1);   // this CTA's dS^T buffer is complete
           mbar_wait(bar_ds_full + 8 * b, (q >> 1) & 1);   // ... and the peer's
           fence_proxy_async_smem();
-          if (q + 1 < n_iters) mbar_wait(bar_dpr + 8 * (b ^ 1), ((q + 1) >> 1) & 1);               // S^T(q+1) has been read
+          if (q + 1 < n_iters) mbar_wait(bar_dpr + 8 * (b ^ 1), ((q + 1) >> 1) & 1);               // columns [0,32) of S^T(q+1) (the first parts) have been read
           else if (q >= 2) mbar_wait(bar_dq_empty + 8 * b, ((q - 2) >> 1) & 1);                      // last tile: dQ^T(q-2) drained
           tc_fence_after();
           SAP_STAMP2(q, 12);
@@ -280,23 +285,24 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
           SAP_STAMP2(q, 4);
         }
         if (j < n_iters) {
-          const int bj = j & 1, stj = j % kPairStages;
           mbar_wait(bar_qm_full + 8 * stj, (j / kPairStages) & 1);
+          mbar_wait(bar_p_full + 8 * bj, (j >> 1) & 1);
+          tc_fence_after();
           SAP_STAMP2(j, 15);
-          const uint32_t tPT = tBuf + 128 * bj + 64;
-          const uint64_t dqm = desc_add(dQm0, stj * L::kQBytes), ddom = desc_add(dDOm0, stj * L::kQBytes);
-          // k = 16 q rows = one column part; every compute warp finishes its first part (k even) well before its second
 #pragma unroll
-          for (int pp = 0; pp < 2; ++pp) {
-            mbar_wait((pp ? bar_p_full2 : bar_p_full) + 8 * bj, (j >> 1) & 1);
-            tc_fence_after();
+          for (int k = 0; k < 2; ++k)   // k = 16 q rows = one column part
+            umma2_ts(tDV, tPT + k * 16, desc_add(ddom, k * 2048), idesc_acc, (j > 0 || k > 0) ? 1u : 0u);
 #pragma unroll
-            for (int k = pp; k < kBwdN / 16; k += 2)
-              umma2_ts(tDV, tPT + k * 16, desc_add(ddom, k * 2048), idesc_acc, (j > 0 || k > 0) ? 1u : 0u);
+          for (int k = 0; k < 2; ++k)
+            umma2_ts(tDK, tPT + k * 16 + 8, desc_add(dqm, k * 2048), idesc_acc, (j > 0 || k > 0) ? 1u : 0u);
+          mbar_wait(bar_p_full2 + 8 * bj, (j >> 1) & 1);
+          tc_fence_after();
 #pragma unroll
-            for (int k = pp; k < kBwdN / 16; k += 2)
-              umma2_ts(tDK, tPT + k * 16 + 8, desc_add(dqm, k * 2048), idesc_acc, (j > 0 || k > 0) ? 1u : 0u);
-          }
+          for (int k = 2; k < kBwdN / 16; ++k)
+            umma2_ts(tDV, tPT + k * 16, desc_add(ddom, k * 2048), idesc_acc, 1u);
+#pragma unroll
+          for (int k = 2; k < kBwdN / 16; ++k)
+            umma2_ts(tDK, tPT + k * 16 + 8, desc_add(dqm, k * 2048), idesc_acc, 1u);
           umma2_commit(bar_qm_empty + 8 * stj, 3);
           umma2_commit(bar_dvk_done + 8 * bj, 1);
           SAP_STAMP2(j, 3);
@@ -309,7 +315,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
     const int quarter = warp & 3, dpart = (warp - 4 - 4 * kFusedParts) >> 2;
     constexpr int kCols = 32 / kFusedDrainGroups;          // TMEM columns (q rows) per drain warp
     const int dcol = 64 * static_cast<int>(cta) + 32 * (quarter & 1) + lane;  // d index of this TMEM lane
-    const int qoff = 32 * (quarter >> 1) + kCols * dpart;                     // first q row of this warp's columns
+    const int qoff = 16 * (2 * dpart + (quarter >> 1));                       // first q row of this warp's 16 columns: N half h = lane / 64 holds q rows [16 h, +16) and [32 + 16 h, +16)
     const uint32_t lane_base = static_cast<uint32_t>(quarter * 32) << 16;
     const size_t row_stride = static_cast<size_t>(n_q_heads) * D;
     const uint32_t lead_dq_empty = mapa_cluster(bar_dq_empty, 0);
@@ -361,12 +367,13 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
     // 64-byte swizzle (chunk ^= bits 7-8 of the byte offset)
     const uint32_t prow = static_cast<uint32_t>(kTile * cta + r) * 64, psw = ((prow >> 7) & 3) << 4;
     const uint32_t ds_dst = mapa_cluster(sDS, static_cast<uint32_t>(qh));
-    const uint32_t lead_p_full = mapa_cluster(bar_p_full, 0), lead_p_full2 = mapa_cluster(bar_p_full2, 0), lead_dpr = mapa_cluster(bar_dpr, 0);
+    const uint32_t lead_p_full = mapa_cluster(bar_p_full, 0), lead_p_full2 = mapa_cluster(bar_p_full2, 0), lead_dpr = mapa_cluster(bar_dpr, 0), lead_dpr2 = mapa_cluster(bar_dpr2, 0);
     const uint32_t peer_ds_land = mapa_cluster(bar_ds_land, cta ^ 1);
     const bool ds_expect = quarter == 0;   // one of the 4 local-storing warps of a tile announces the peer's bytes
     uint8_t* const ds_local = (static_cast<uint32_t>(qh) == cta) ? smem + L::kOffDS : nullptr;  // own q half: plain stores
     const int b = group;
-    const uint32_t tS0 = tBuf + 128 * b + lane_base + 2 * kFusedCols * qh;
+    const uint64_t scale2 = pack_f32x2(scale_log2, scale_log2);
+    const uint32_t tS0 = tBuf + 128 * b + lane_base + kFusedCols * qh;
 
     int i = 0;
     for (int hq = 0; hq < g; ++hq) {
@@ -385,8 +392,8 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
           uint32_t dsk[2][kFusedCols / 2];
 #pragma unroll
           for (int pp = 0; pp < 2; ++pp) {
-            const int part = 2 * qh + pp;
-            const uint32_t tST = tS0 + kFusedCols * pp, tDPT = tST + 64;
+            const int part = 2 * pp + qh;   // first parts = q rows [0,32), second parts = [32,64): columns [0,32) of S^T are free for dQ^T early
+            const uint32_t tST = tS0 + 2 * kFusedCols * pp, tDPT = tST + 64;
             const int tc = t0 + kFusedCols * part;  // first q row of this column part
             const bool need_mask = __any_sync(0xffffffffu, (tc < lo) || (tc + kFusedCols > hi));
             uint32_t sv[kFusedCols], dp[kFusedCols];
@@ -398,7 +405,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
             if (warp == 4 && lane == 0 && pp == 0) SAP_STAMP2(i, 23);
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster_relaxed(lead_dpr + 8 * b);   // S^T and dP^T of this part are in registers: the S^T columns may take dQ^T(i-1).  (Both CTAs arrive through the cluster window: no branch on the CTA rank)
+            if (lane == 0) mbar_arrive_cluster_relaxed((pp ? lead_dpr2 : lead_dpr) + 8 * b);   // S^T and dP^T of this part are in registers: the S^T columns may take dQ^T(i-1).  (Both CTAs arrive through the cluster window: no branch on the CTA rank)
             if (lane == 0) { SAP_STAMP_MAX(i, 22); }
             if (need_mask) {  // boundary tiles only: masked scores become -inf, so P = 2^-inf = 0 and dS = 0
 #pragma unroll
@@ -410,18 +417,20 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
             uint32_t pk[kFusedCols];   // P^T (8 words) then dS^T (8 words): 16 TMEM columns
 #pragma unroll
             for (int q4 = 0; q4 < kFusedCols / 4; ++q4) {
-              const float4 lv = l4[q4], dvv = d4[q4];
-              const float ls[4] = {lv.x, lv.y, lv.z, lv.w}, dd[4] = {dvv.x, dvv.y, dvv.z, dvv.w};
-              float pe[4], ds[4];
+              const float4 lv = l4[q4], dvv = d4[q4];   // -LSE and -D of four q rows
+              const uint64_t nl[2] = {pack_f32x2(lv.x, lv.y), pack_f32x2(lv.z, lv.w)};
+              const uint64_t nd[2] = {pack_f32x2(dvv.x, dvv.y), pack_f32x2(dvv.z, dvv.w)};
 #pragma unroll
-              for (int e = 0; e < 4; ++e) {
-                const int idx = q4 * 4 + e;
-                pe[e] = ex2_approx(fmaf(__uint_as_float(sv[idx]), scale_log2, -ls[e]));
-                ds[e] = pe[e] * (__uint_as_float(dp[idx]) - dd[e]);
+              for (int e = 0; e < 2; ++e) {   // two q rows per packed instruction
+                const int idx = q4 * 4 + 2 * e;
+                float x0, x1;
+                unpack_f32x2(fma_f32x2(pack_f32x2(__uint_as_float(sv[idx]), __uint_as_float(sv[idx + 1])), scale2, nl[e]), x0, x1);
+                const float p0 = ex2_approx(x0), p1 = ex2_approx(x1);
+                float s0, s1;
+                unpack_f32x2(mul_f32x2(pack_f32x2(p0, p1), add_f32x2(pack_f32x2(__uint_as_float(dp[idx]), __uint_as_float(dp[idx + 1])), nd[e])), s0, s1);
+                pk[q4 * 2 + e] = pack_bf16x2(p0, p1);
+                pk[kFusedCols / 2 + q4 * 2 + e] = dsk[pp][q4 * 2 + e] = pack_bf16x2(s0, s1);
               }
-              pk[q4 * 2] = pack_bf16x2(pe[0], pe[1]); pk[q4 * 2 + 1] = pack_bf16x2(pe[2], pe[3]);
-              pk[kFusedCols / 2 + q4 * 2] = dsk[pp][q4 * 2] = pack_bf16x2(ds[0], ds[1]);
-              pk[kFusedCols / 2 + q4 * 2 + 1] = dsk[pp][q4 * 2 + 1] = pack_bf16x2(ds[2], ds[3]);
             }
             if (warp == 4 && lane == 0 && pp == 0) SAP_STAMP2(i, 24);
             tmem_st16(tDPT, pk);  // bf16 P^T and dS^T over the 16 dP^T columns just read
