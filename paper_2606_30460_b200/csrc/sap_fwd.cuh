@@ -233,7 +233,9 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
         }
         const float neg_m = (m_used == -CUDART_INF_F) ? 0.f : -m_used;
         // P = 2^(S*scale_log2 - m) (masked entries: 2^-inf = 0), row sum, bf16 P back into TMEM over S
-        float ls4[4] = {0.f, 0.f, 0.f, 0.f};
+        // packed fp32 pairs (FFMA2 / FADD2): the two softmax warps of a scheduler are issue-bound, not MUFU-bound
+        const uint64_t sc2 = pack_f32x2(scale_log2, scale_log2), nm2 = pack_f32x2(neg_m, neg_m);
+        uint64_t ls2[4] = {0ull, 0ull, 0ull, 0ull};   // four pairs of partial row sums
 #pragma unroll
         for (int half = 0; half < 2; ++half) {
 #pragma unroll
@@ -241,9 +243,10 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
             uint32_t pk[16];
 #pragma unroll
             for (int i = 0; i < 32; i += 2) {
-              const float p0 = ex2_approx(fmaf(__uint_as_float(sv[c * 32 + i]), scale_log2, neg_m));
-              const float p1 = ex2_approx(fmaf(__uint_as_float(sv[c * 32 + i + 1]), scale_log2, neg_m));
-              ls4[(i >> 1) & 3] += p0 + p1;
+              float x0, x1;
+              unpack_f32x2(fma_f32x2(pack_f32x2(__uint_as_float(sv[c * 32 + i]), __uint_as_float(sv[c * 32 + i + 1])), sc2, nm2), x0, x1);
+              const float p0 = ex2_approx(x0), p1 = ex2_approx(x1);
+              ls2[(i >> 1) & 3] = add_f32x2(ls2[(i >> 1) & 3], pack_f32x2(p0, p1));
               pk[i >> 1] = pack_bf16x2(p0, p1);
             }
             tmem_st16(tP + lane_base + c * 16, pk);
@@ -252,7 +255,11 @@ sap_fwd_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__
           tc_fence_before();
           mbar_arrive(bar_p_full + 8 * half);
         }
-        l_run += (ls4[0] + ls4[1]) + (ls4[2] + ls4[3]);
+        {
+          float a0, a1;
+          unpack_f32x2(add_f32x2(add_f32x2(ls2[0], ls2[1]), add_f32x2(ls2[2], ls2[3])), a0, a1);
+          l_run += a0 + a1;
+        }
       }
     }
     // ---- epilogue: O / l -> global, LSE (natural log, PAPER.md silent: SURVEY A-11)

@@ -231,7 +231,9 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
           }
         }
         const float neg_m = (m_used == -CUDART_INF_F) ? 0.f : -m_used;
-        float ls4[4] = {0.f, 0.f, 0.f, 0.f};
+        // packed fp32 pairs (FFMA2 / FADD2): the two softmax warps of a scheduler are issue-bound, not MUFU-bound
+        const uint64_t sc2 = pack_f32x2(scale_log2, scale_log2), nm2 = pack_f32x2(neg_m, neg_m);
+        uint64_t ls2[4] = {0ull, 0ull, 0ull, 0ull};   // four pairs of partial row sums
 #pragma unroll
         for (int half = 0; half < 2; ++half) {
 #pragma unroll
@@ -239,9 +241,10 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
             uint32_t pk[16];
 #pragma unroll
             for (int i = 0; i < 32; i += 2) {
-              const float p0 = ex2_approx(fmaf(__uint_as_float(sv[c * 32 + i]), scale_log2, neg_m));
-              const float p1 = ex2_approx(fmaf(__uint_as_float(sv[c * 32 + i + 1]), scale_log2, neg_m));
-              ls4[(i >> 1) & 3] += p0 + p1;
+              float x0, x1;
+              unpack_f32x2(fma_f32x2(pack_f32x2(__uint_as_float(sv[c * 32 + i]), __uint_as_float(sv[c * 32 + i + 1])), sc2, nm2), x0, x1);
+              const float p0 = ex2_approx(x0), p1 = ex2_approx(x1);
+              ls2[(i >> 1) & 3] = add_f32x2(ls2[(i >> 1) & 3], pack_f32x2(p0, p1));
               pk[i >> 1] = pack_bf16x2(p0, p1);
             }
             tmem_st16(tP + lane_base + c * 16, pk);
@@ -251,7 +254,11 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
           mbar_arrive(bar_p + 8 * half);
           if ((warp & 3) == 0 && lane == 0) FWD_STAMP(it, 17 + 8 * x + half);
         }
-        l_run += (ls4[0] + ls4[1]) + (ls4[2] + ls4[3]);
+        {
+          float a0, a1;
+          unpack_f32x2(add_f32x2(add_f32x2(ls2[0], ls2[1]), add_f32x2(ls2[2], ls2[3])), a0, a1);
+          l_run += a0 + a1;
+        }
       }
     }
     // ---- epilogue: O / l -> global, LSE (natural log)
