@@ -70,12 +70,22 @@ static cudaError_t set_kernel_attributes() {
   return cudaSuccess;
 }
 
+// Per-device state of the persistent kernels: the SM count and a pool of {next, done} counter pairs (zero between
+// launches: the last CTA of a launch re-arms its pair).  Launches take the pairs round-robin, so kernels that run
+// concurrently on different streams do not share one unless more than kSchedSlots are in flight at once.
+constexpr int kSchedSlots = 64;
+struct DeviceSched { int n_sms = 0; int* pool = nullptr; std::atomic<unsigned> seq{0}; };
+static DeviceSched g_sched[64];
+
+static int* next_sched_pair(int dev) { return g_sched[dev].pool + 2 * (g_sched[dev].seq.fetch_add(1) % kSchedSlots); }
+
 int ensure_device(int* dev_out) {
   static std::mutex mu;
   static std::set<int> ready, wrong_arch;
   int dev = 0;
   SAP_CUDA_CHECK(cudaGetDevice(&dev));
   if (dev_out) *dev_out = dev;
+  if (dev < 0 || dev >= 64) return SAP_ERR_UNSUPPORTED;
   std::lock_guard<std::mutex> lock(mu);
   if (ready.count(dev)) return SAP_OK;
   if (wrong_arch.count(dev)) return SAP_ERR_WRONG_ARCH;
@@ -85,6 +95,11 @@ int ensure_device(int* dev_out) {
   SAP_CUDA_CHECK(set_kernel_attributes<64>());
   SAP_CUDA_CHECK(set_kernel_attributes<128>());
   SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PairSmem::kTotal));
+  SAP_CUDA_CHECK(cudaDeviceGetAttribute(&g_sched[dev].n_sms, cudaDevAttrMultiProcessorCount, dev));
+  if (!g_sched[dev].pool) {
+    SAP_CUDA_CHECK(cudaMalloc(&g_sched[dev].pool, 2 * kSchedSlots * sizeof(int)));
+    SAP_CUDA_CHECK(cudaMemset(g_sched[dev].pool, 0, 2 * kSchedSlots * sizeof(int)));
+  }
   ready.insert(dev);
   return SAP_OK;
 }
@@ -159,10 +174,14 @@ static int launch_fwd(const DevProgram& prog, const void* q, const void* k, cons
   if ((rc = make_tile_map(&mk, k, plan->n_tokens, (int64_t)Hkv * D)) != SAP_OK) return rc;
   if ((rc = make_tile_map(&mv, v, plan->n_tokens, (int64_t)Hkv * D)) != SAP_OK) return rc;
   if ((Hq / Hkv) % 2 == 0 && g_fwd_form.load() == 0) {  // two q-heads of a GQA group per CTA share the K/V stream
-    const unsigned grid = static_cast<unsigned>(prog.n_tiles) * (Hq / 2);
+    // persistent: one CTA per SM, work items handed out in launch order (kv-head-major, longest tile first)
+    int dev = 0;
+    SAP_CUDA_CHECK(cudaGetDevice(&dev));
+    const int n_work = prog.n_tiles * (Hq / 2);
+    const unsigned grid = static_cast<unsigned>(n_work < g_sched[dev].n_sms ? n_work : g_sched[dev].n_sms);
     sap_fwd_pair_kernel<D, PARTIAL><<<grid, kFwdPairThreads, FwdPairSmem<D>::kTotal, stream>>>(
         mq, mk, mv, prog.tiles, prog.segs, cu, plan->n_docs, static_cast<__nv_bfloat16*>(out), out_f32, lse,
-        plan->n_tokens, Hq, Hkv, scale * kLog2e);
+        plan->n_tokens, Hq, Hkv, scale * kLog2e, prog.n_tiles, n_work, next_sched_pair(dev));
   } else {
     const unsigned grid = static_cast<unsigned>(prog.n_tiles) * Hq;
     sap_fwd_kernel<D, PARTIAL><<<grid, kFwdThreads, FwdSmem<D>::kTotal, stream>>>(

@@ -134,11 +134,12 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
                      lead_qm_full = mapa_cluster(bar_qm_full, 0);
       const int dcol = hk * D + 64 * static_cast<int>(cta);  // this CTA's d half
       if (cta == 0) mbar_expect_tx(bar_kv_full, L::kKVTxBytes);
+      const uint64_t pol_once = l2_policy_evict_first();   // a pair's own K / V tiles are read by nobody else
 #pragma unroll
       for (int b = 0; b < 2; ++b) {
-        tma_load_2d_pair(sK + b * L::kKVBox, &mapK, hk * D + b * 64, key0, lead_kv_full);
-        tma_load_2d_pair(sV + b * L::kKVBox, &mapV, hk * D + b * 64, key0, lead_kv_full);
-        tma_load_2d_pair(sKT + b * L::kKVBox, &mapK, dcol, td.row0 + b * kTile, lead_kv_full);  // both key tiles, own d half
+        tma_load_2d_pair_hint(sK + b * L::kKVBox, &mapK, hk * D + b * 64, key0, lead_kv_full, pol_once);
+        tma_load_2d_pair_hint(sV + b * L::kKVBox, &mapV, hk * D + b * 64, key0, lead_kv_full, pol_once);
+        tma_load_2d_pair_hint(sKT + b * L::kKVBox, &mapK, dcol, td.row0 + b * kTile, lead_kv_full, pol_once);  // both key tiles, own d half
       }
       // the d-half slots of a tile are needed more than a tile later than its q-half slots: load them one tile behind,
       // so that waiting for their ring never holds back the next q-half loads
@@ -319,6 +320,7 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
     const uint32_t lane_base = static_cast<uint32_t>(quarter * 32) << 16;
     const size_t row_stride = static_cast<size_t>(n_q_heads) * D;
     const uint32_t lead_dq_empty = mapa_cluster(bar_dq_empty, 0);
+    const uint64_t pol_acc = l2_policy_evict_last();   // accumulator lines: a miss is a DRAM read plus a write-back
     int j = 0;
     for (int hq = 0; hq < g; ++hq) {
       const int h = hk * g + hq;
@@ -340,11 +342,11 @@ sap_bwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ32, const __grid_con
           if (warp == 4 + 4 * kFusedParts && lane == 0) SAP_STAMP2(j, 9);
           if (tq + kCols <= n_tokens) {
 #pragma unroll
-            for (int c = 0; c < kCols; ++c) { red_add_f32(dst, __uint_as_float(v[c])); dst += row_stride; }
+            for (int c = 0; c < kCols; ++c) { red_add_f32_hint(dst, __uint_as_float(v[c]), pol_acc); dst += row_stride; }
           } else {
 #pragma unroll
             for (int c = 0; c < kCols; ++c) {
-              if (tq + c < n_tokens) red_add_f32(dst, __uint_as_float(v[c]));
+              if (tq + c < n_tokens) red_add_f32_hint(dst, __uint_as_float(v[c]), pol_acc);
               dst += row_stride;
             }
           }

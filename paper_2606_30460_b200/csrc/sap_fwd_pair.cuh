@@ -1,4 +1,6 @@
-// Forward kernel, pair form: one CTA = one 128-row Q tile x TWO q-heads of one GQA group, one CTA per SM.
+// Forward kernel, pair form: one work item = one 128-row Q tile x TWO q-heads of one GQA group; PERSISTENT: one CTA per
+// SM takes work items off a global counter in the launch order (kv-head-major, longest tile first), so barriers, TMEM
+// and the K/V ring are set up once and the next item's Q / first K/V loads and first S run under the current item's tail.
 // (`computing` of PAPER.md Table 1 (:85-98) with the "copy and rescale" merge (:239) fused, as in sap_fwd.cuh.)
 //
 // The two heads attend the same rows to the same keys, so they walk the same segments and share every K / V tile
@@ -34,13 +36,30 @@ struct FwdPairSmem {
   static constexpr int kTotal = kBarOffset + 256;
 };
 
+// Work item w of a launch -> (kv-head, Q tile, first q-head of the pair): kv-head-major, tiles longest-first inside a
+// head, the g/2 head pairs of a tile adjacent (CTAs that run side by side share one kv-head's K/V in L2).
+struct FwdPairWork { int hk, tile_idx, h0; };
+__device__ __forceinline__ FwdPairWork fwd_pair_work(int w, int n_tiles, int g) {
+  const int pairs = g / 2, per_head = n_tiles * pairs;
+  const int hk = w / per_head, rem = w % per_head;
+  return {hk, rem / pairs, hk * g + 2 * (rem % pairs)};
+}
+__device__ __forceinline__ int fwd_tile_iters(const TileDesc& td, const SegDesc* __restrict__ segs) {
+  int n = 0;
+  for (int s = td.seg_begin; s < td.seg_end; ++s) n += (segs[s].t_end - segs[s].t_begin + kTile - 1) / kTile;
+  return n;
+}
+
+// `sched` = {next, done}: two zero-initialised counters of this launch.  CTA b starts with item b and then takes item
+// gridDim.x + atomicAdd(next, 1); the last CTA to leave zeroes both again, so the pair can serve the next launch.
 template <int D, bool PARTIAL>
 __global__ void __launch_bounds__(kFwdPairThreads, 1)
 sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
                     const __grid_constant__ CUtensorMap mapV, const TileDesc* __restrict__ tiles,
                     const SegDesc* __restrict__ segs, const int32_t* __restrict__ cu, int n_docs,
                     __nv_bfloat16* __restrict__ out, float* __restrict__ out_f32, float* __restrict__ lse,
-                    int n_tokens, int n_q_heads, int n_kv_heads, float scale_log2) {
+                    int n_tokens, int n_q_heads, int n_kv_heads, float scale_log2, int n_tiles, int n_work,
+                    int* __restrict__ sched) {
   using L = FwdPairSmem<D>;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = smem_raw;
@@ -49,28 +68,29 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
   const uint32_t sQ = s0 + L::kOffQ, sK = s0 + L::kOffK, sV = s0 + L::kOffV;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L::kBarOffset);
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kBarOffset + 240);
+  volatile int* work_ring = reinterpret_cast<volatile int*>(smem + L::kBarOffset + 224);   // 2 slots
   const uint32_t bar_q_full = smem_u32(bars + 0), bar_k_full = smem_u32(bars + 1), bar_k_empty = smem_u32(bars + 3),
                  bar_v_full = smem_u32(bars + 5), bar_v_empty = smem_u32(bars + 7),
                  bar_s_full = smem_u32(bars + 9) /* [A, B] */, bar_p_full = smem_u32(bars + 11) /* [A0, A1, B0, B1] */,
-                 bar_o_full = smem_u32(bars + 15) /* [A, B] */;
+                 bar_o_full = smem_u32(bars + 15) /* [A, B] */, bar_q_empty = smem_u32(bars + 17),
+                 bar_o_empty = smem_u32(bars + 18) /* [A, B] */, bar_w_full = smem_u32(bars + 20) /* [2] */,
+                 bar_w_empty = smem_u32(bars + 22) /* [2] */;
 
   // logical warp id: the service warpgroup (logical warps 0-3) is the physically last one (see sap_fwd.cuh)
   const int warp = ((threadIdx.x >> 5) + 4) % (kFwdPairThreads / 32), lane = threadIdx.x & 31;
-  // grid order: kv-head-major, tiles longest-first inside a head, the g/2 head pairs of a tile adjacent
-  const int g = n_q_heads / n_kv_heads, pairs = g / 2;
-  const int per_head = (gridDim.x / (n_kv_heads * pairs)) * pairs;
-  const int hk = blockIdx.x / per_head, rem = blockIdx.x % per_head;
-  const int tile_idx = rem / pairs, h0 = hk * g + 2 * (rem % pairs);  // heads h0 (A) and h0 + 1 (B)
-  const TileDesc td = tiles[tile_idx];
+  const int g = n_q_heads / n_kv_heads;
 
   if (threadIdx.x == 0) {
-    mbar_init(bar_q_full, 1);
+    mbar_init(bar_q_full, 1); mbar_init(bar_q_empty, 1);
     for (int i = 0; i < kFwdPairStages; ++i) {
       mbar_init(bar_k_full + 8 * i, 1); mbar_init(bar_k_empty + 8 * i, 1);
       mbar_init(bar_v_full + 8 * i, 1); mbar_init(bar_v_empty + 8 * i, 1);
     }
-    for (int i = 0; i < 2; ++i) { mbar_init(bar_s_full + 8 * i, 1); mbar_init(bar_o_full + 8 * i, 1); }
-    for (int i = 0; i < 4; ++i) mbar_init(bar_p_full + 8 * i, 128);
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(bar_s_full + 8 * i, 1); mbar_init(bar_o_full + 8 * i, 1); mbar_init(bar_o_empty + 8 * i, 4);
+      mbar_init(bar_w_full + 8 * i, 1); mbar_init(bar_w_empty + 8 * i, 1 + 8);   // issuer + 8 softmax warps
+    }
+    for (int i = 0; i < 4; ++i) mbar_init(bar_p_full + 8 * i, 4);   // one arrival per softmax warp
     fence_mbar_init();
     tma_prefetch_desc(&mapQ); tma_prefetch_desc(&mapK); tma_prefetch_desc(&mapV);
   }
@@ -80,41 +100,52 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
   tc_fence_after();
   const uint32_t tmem = *tmem_slot;
 
-  int n_iters = 0;
-  for (int s = td.seg_begin; s < td.seg_end; ++s) n_iters += (segs[s].t_end - segs[s].t_begin + kTile - 1) / kTile;
-
   if (warp < 4) {
-    reg_dealloc<72>();
+    reg_dealloc<88>();
     if (warp == 0) {
-      // ---------------------------------------------------------------- TMA producer
-      if (n_iters > 0 && elect_one()) {
-        mbar_expect_tx(bar_q_full, 2 * L::kTileBytes);
+      // ---------------------------------------------------------------- scheduler + TMA producer
+      if (elect_one()) {
+        int st = 0, ph = 1;  // K/V rings run on across work items; empty barriers: the first pass must not block
+        int ws = 0, wph = 1, nq = 0;   // work ring slot / phase; items with loads so far
+        for (int w = blockIdx.x;; w = gridDim.x + atomicAdd(sched, 1)) {
+          const bool end = w >= n_work;
+          mbar_wait(bar_w_empty + 8 * ws, wph);
+          work_ring[ws] = end ? -1 : w;
+          mbar_arrive(bar_w_full + 8 * ws);   // release: the slot is written
+          if (++ws == 2) { ws = 0; wph ^= 1; }
+          if (end) break;
+          const FwdPairWork wk = fwd_pair_work(w, n_tiles, g);
+          const TileDesc td = tiles[wk.tile_idx];
+          if (fwd_tile_iters(td, segs) == 0) continue;
+          mbar_wait(bar_q_empty, (nq & 1) ^ 1);   // the last S of the previous item has read Q
+          ++nq;
+          mbar_expect_tx(bar_q_full, 2 * L::kTileBytes);
 #pragma unroll
-        for (int x = 0; x < 2; ++x)
-#pragma unroll
-          for (int b = 0; b < L::kBoxes; ++b)
-            tma_load_2d(sQ + x * L::kTileBytes + b * L::kBoxBytes, &mapQ, (h0 + x) * D + b * 64, td.row0, bar_q_full);
-        int st = 0, ph = 1;  // empty barriers: the first pass over the rings must not block
-        for (int s = td.seg_begin; s < td.seg_end; ++s) {
-          const int c_begin = segs[s].t_begin, c_end = segs[s].t_end;
-          for (int c0 = c_begin; c0 < c_end; c0 += kTile) {
-            mbar_wait(bar_k_empty + 8 * st, ph);
-            mbar_expect_tx(bar_k_full + 8 * st, L::kTileBytes);
+          for (int x = 0; x < 2; ++x)
 #pragma unroll
             for (int b = 0; b < L::kBoxes; ++b)
-              tma_load_2d(sK + st * L::kTileBytes + b * L::kBoxBytes, &mapK, hk * D + b * 64, c0, bar_k_full + 8 * st);
-            mbar_wait(bar_v_empty + 8 * st, ph);
-            mbar_expect_tx(bar_v_full + 8 * st, L::kTileBytes);
+              tma_load_2d(sQ + x * L::kTileBytes + b * L::kBoxBytes, &mapQ, (wk.h0 + x) * D + b * 64, td.row0, bar_q_full);
+          for (int s = td.seg_begin; s < td.seg_end; ++s) {
+            const int c_begin = segs[s].t_begin, c_end = segs[s].t_end;
+            for (int c0 = c_begin; c0 < c_end; c0 += kTile) {
+              mbar_wait(bar_k_empty + 8 * st, ph);
+              mbar_expect_tx(bar_k_full + 8 * st, L::kTileBytes);
 #pragma unroll
-            for (int b = 0; b < L::kBoxes; ++b)
-              tma_load_2d(sV + st * L::kTileBytes + b * L::kBoxBytes, &mapV, hk * D + b * 64, c0, bar_v_full + 8 * st);
-            if (++st == kFwdPairStages) { st = 0; ph ^= 1; }
+              for (int b = 0; b < L::kBoxes; ++b)
+                tma_load_2d(sK + st * L::kTileBytes + b * L::kBoxBytes, &mapK, wk.hk * D + b * 64, c0, bar_k_full + 8 * st);
+              mbar_wait(bar_v_empty + 8 * st, ph);
+              mbar_expect_tx(bar_v_full + 8 * st, L::kTileBytes);
+#pragma unroll
+              for (int b = 0; b < L::kBoxes; ++b)
+                tma_load_2d(sV + st * L::kTileBytes + b * L::kBoxBytes, &mapV, wk.hk * D + b * 64, c0, bar_v_full + 8 * st);
+              if (++st == kFwdPairStages) { st = 0; ph ^= 1; }
+            }
           }
         }
       }
     } else if (warp == 1) {
       // ---------------------------------------------------------------- tcgen05 issuer (one elected thread)
-      if (n_iters > 0 && elect_one()) {
+      if (elect_one()) {
         constexpr uint32_t idesc_s = make_idesc_bf16(128, 128, 0, 0);  // S[128x128] = Q (K-major) x K^T (K-major)
         constexpr uint32_t idesc_o = make_idesc_bf16(128, D, 0, 1);    // O[128xD]  = P (TMEM)   x V (MN-major)
         auto issue_s = [&](int x, int st) {   // S_x = Q_x K^T for the K tile in stage st
@@ -126,186 +157,224 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
           }
           umma_commit(bar_s_full + 8 * x);
         };
-        auto issue_pv = [&](int x, int st, int it) {  // O_x += P_x V, in two halves of 64 keys
+        int st = 0, ph = 0;   // stage / phase of the current iteration; run on across work items
+        int gi = 0;           // iterations so far (parity of the P barriers)
+        int nq = 0;           // items with work so far (parity of the Q / O barriers)
+        int ws = 0, wph = 0;
+        for (;;) {
+          mbar_wait(bar_w_full + 8 * ws, wph);
+          const int w = work_ring[ws];
+          mbar_arrive(bar_w_empty + 8 * ws);
+          if (++ws == 2) { ws = 0; wph ^= 1; }
+          if (w < 0) break;
+          const FwdPairWork wk = fwd_pair_work(w, n_tiles, g);
+          const int n_iters = fwd_tile_iters(tiles[wk.tile_idx], segs);
+          if (n_iters == 0) continue;
+          auto issue_pv = [&](int x, int st_, int it) {  // O_x += P_x V, in two halves of 64 keys
 #pragma unroll
-          for (int half = 0; half < 2; ++half) {
-            mbar_wait(bar_p_full + 8 * (2 * x + half), it & 1);
-            tc_fence_after();
+            for (int half = 0; half < 2; ++half) {
+              mbar_wait(bar_p_full + 8 * (2 * x + half), gi & 1);
+              tc_fence_after();
 #pragma unroll
-            for (int k = half * 4; k < half * 4 + 4; ++k)  // 16 keys per MMA: 2 groups of 8 rows (SBO 1024 B)
-              umma_ts(tmem + 256 + 128 * x, tmem + 128 * x + k * 8,
-                      make_smem_desc(sV + st * L::kTileBytes + k * 2048, L::kBoxBytes, 1024), idesc_o,
-                      (it > 0 || k > 0) ? 1u : 0u);
-          }
-          if (it == n_iters - 1) umma_commit(bar_o_full + 8 * x);
-        };
-        mbar_wait(bar_q_full, 0);
-        mbar_wait(bar_k_full, 0);
-        tc_fence_after();
-        issue_s(0, 0);
-        issue_s(1, 0);
-        umma_commit(bar_k_empty);
-        int st = 0, ph = 0;  // stage / phase of iteration `it`
-        for (int it = 0; it < n_iters; ++it) {
-          const int st_n = (st + 1 == kFwdPairStages) ? 0 : st + 1, ph_n = (st_n == 0) ? ph ^ 1 : ph;
-          const bool more = it + 1 < n_iters;
-          FWD_STAMP(it, 0);
-          mbar_wait(bar_v_full + 8 * st, ph);
-          FWD_STAMP(it, 1);
-          issue_pv(0, st, it);
-          FWD_STAMP(it, 2);
-          if (more) {
-            mbar_wait(bar_k_full + 8 * st_n, ph_n);
+              for (int k = half * 4; k < half * 4 + 4; ++k)  // 16 keys per MMA: 2 groups of 8 rows (SBO 1024 B)
+                umma_ts(tmem + 256 + 128 * x, tmem + 128 * x + k * 8,
+                        make_smem_desc(sV + st_ * L::kTileBytes + k * 2048, L::kBoxBytes, 1024), idesc_o,
+                        (it > 0 || k > 0) ? 1u : 0u);
+            }
+            if (it == n_iters - 1) umma_commit(bar_o_full + 8 * x);
+          };
+          mbar_wait(bar_q_full, nq & 1);
+          mbar_wait(bar_k_full + 8 * st, ph);
+          tc_fence_after();
+          issue_s(0, st);
+          issue_s(1, st);
+          umma_commit(bar_k_empty + 8 * st);
+          if (n_iters == 1) umma_commit(bar_q_empty);   // the item's last S has been issued: Q may be overwritten once it is done
+          if (nq > 0) {   // the previous item's O_A, O_B have left TMEM (long before the first P of this item is ready)
+            mbar_wait(bar_o_empty, (nq - 1) & 1);
+            mbar_wait(bar_o_empty + 8, (nq - 1) & 1);
             tc_fence_after();
-            issue_s(0, st_n);   // S_A(it+1) runs while warpgroup B is still in softmax_B(it)
           }
-          FWD_STAMP(it, 3);
-          issue_pv(1, st, it);
-          FWD_STAMP(it, 4);
-          umma_commit(bar_v_empty + 8 * st);
-          if (more) {
-            issue_s(1, st_n);
-            umma_commit(bar_k_empty + 8 * st_n);
+          for (int it = 0; it < n_iters; ++it, ++gi) {
+            const int st_n = (st + 1 == kFwdPairStages) ? 0 : st + 1, ph_n = (st_n == 0) ? ph ^ 1 : ph;
+            const bool more = it + 1 < n_iters;
+            FWD_STAMP(it, 0);
+            mbar_wait(bar_v_full + 8 * st, ph);
+            FWD_STAMP(it, 1);
+            issue_pv(0, st, it);
+            FWD_STAMP(it, 2);
+            if (more) {
+              mbar_wait(bar_k_full + 8 * st_n, ph_n);
+              tc_fence_after();
+              issue_s(0, st_n);   // S_A(it+1) runs while warpgroup B is still in softmax_B(it)
+            }
+            FWD_STAMP(it, 3);
+            issue_pv(1, st, it);
+            FWD_STAMP(it, 4);
+            umma_commit(bar_v_empty + 8 * st);
+            if (more) {
+              issue_s(1, st_n);
+              umma_commit(bar_k_empty + 8 * st_n);
+              if (it + 2 == n_iters) umma_commit(bar_q_empty);
+            }
+            st = st_n; ph = ph_n;
           }
-          st = st_n; ph = ph_n;
+          ++nq;
         }
       }
     }
   } else {
     // ------------------------------------------------------------------ softmax / correction / epilogue (A or B)
-    reg_alloc<216>();  // 256 x 216 + 128 x 72 = the 384 x 168 register pool
+    reg_alloc<208>();  // 256 x 208 + 128 x 88 = the 384 x 168 register pool
     const int x = (warp - 4) >> 2;  // 0: head h0 (A), 1: head h0 + 1 (B)
-    const int h = h0 + x;
     const int r = (warp & 3) * 32 + lane;
-    const int t = td.row0 + r;
-    const bool valid = r < td.rows;
     const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t tS = tmem + 128 * x, tP = tS, tO = tmem + 256 + 128 * x;
-    const uint32_t bar_s = bar_s_full + 8 * x, bar_p = bar_p_full + 16 * x, bar_o = bar_o_full + 8 * x;
-    const int32_t doc_lo = valid ? doc_start_of(cu, n_docs, t) : 0;
-    float m_used = -CUDART_INF_F;  // reference max (log2 domain) the running sum and O are scaled by
-    float l_run = 0.f;
-    int it = 0;
-    for (int s = td.seg_begin; s < td.seg_end; ++s) {
-      const SegDesc sd = segs[s];
-      int lo = max(doc_lo, sd.kv_lo), hi = min(t + 1, sd.kv_hi);  // visible keys of this row: [lo, hi)
-      if (!valid || t < sd.q_lo || t >= sd.q_hi) { lo = 0; hi = 0; }
-      for (int c0 = sd.t_begin; c0 < sd.t_end; c0 += kTile, ++it) {
-        mbar_wait(bar_s, it & 1);
-        tc_fence_after();
-        if ((warp & 3) == 0 && lane == 0) FWD_STAMP(it, 16 + 8 * x);
-        const bool need_mask = __any_sync(0xffffffffu, (c0 < lo) || (c0 + kTile > hi));
-        uint32_t sv[128];  // the whole S row of this thread
+    const uint32_t bar_s = bar_s_full + 8 * x, bar_p = bar_p_full + 16 * x, bar_o = bar_o_full + 8 * x,
+                   bar_oe = bar_o_empty + 8 * x;
+    int gi = 0, nq = 0, ws = 0, wph = 0;
+    for (;;) {
+      mbar_wait(bar_w_full + 8 * ws, wph);
+      const int w = work_ring[ws];
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_w_empty + 8 * ws);
+      if (++ws == 2) { ws = 0; wph ^= 1; }
+      if (w < 0) break;
+      const FwdPairWork wk = fwd_pair_work(w, n_tiles, g);
+      const TileDesc td = tiles[wk.tile_idx];
+      const int n_iters = fwd_tile_iters(td, segs);
+      const int h = wk.h0 + x;
+      const int t = td.row0 + r;
+      const bool valid = r < td.rows;
+      const int32_t doc_lo = valid ? doc_start_of(cu, n_docs, t) : 0;
+      float m_used = -CUDART_INF_F;  // reference max (log2 domain) the running sum and O are scaled by
+      float l_run = 0.f;
+      int it = 0;
+      for (int s = td.seg_begin; s < td.seg_end; ++s) {
+        const SegDesc sd = segs[s];
+        int lo = max(doc_lo, sd.kv_lo), hi = min(t + 1, sd.kv_hi);  // visible keys of this row: [lo, hi)
+        if (!valid || t < sd.q_lo || t >= sd.q_hi) { lo = 0; hi = 0; }
+        for (int c0 = sd.t_begin; c0 < sd.t_end; c0 += kTile, ++it, ++gi) {
+          mbar_wait(bar_s, gi & 1);
+          tc_fence_after();
+          if ((warp & 3) == 0 && lane == 0) FWD_STAMP(it, 16 + 8 * x);
+          const bool need_mask = __any_sync(0xffffffffu, (c0 < lo) || (c0 + kTile > hi));
+          uint32_t sv[128];  // the whole S row of this thread
 #pragma unroll
-        for (int c = 0; c < 4; ++c) tmem_ld32(tS + lane_base + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[c * 32]));
-        tmem_wait_ld();
-        if (need_mask) {  // boundary tiles only (document start, diagonal, item edge)
+          for (int c = 0; c < 4; ++c) tmem_ld32(tS + lane_base + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&sv[c * 32]));
+          tmem_wait_ld();
+          if (need_mask) {  // boundary tiles only (document start, diagonal, item edge)
 #pragma unroll
-          for (int i = 0; i < 128; ++i) {
-            const int col = c0 + i;
-            if (!(col >= lo && col < hi)) sv[i] = 0xff800000u;  // -inf
-          }
-        }
-        float mx4[4] = {-CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F};
-#pragma unroll
-        for (int i = 0; i < 128; i += 4) {
-#pragma unroll
-          for (int e = 0; e < 4; ++e) mx4[e] = fmaxf(mx4[e], __uint_as_float(sv[i + e]));
-        }
-        const float m_new = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * scale_log2;
-        // lazy rescale: only when the max moved by more than 2^8 (or the row saw its first key)
-        const bool grow = m_new > m_used + kRescaleThreshold || (m_used == -CUDART_INF_F && m_new > -CUDART_INF_F);
-        if (__any_sync(0xffffffffu, grow)) {
-          const float f = grow ? ((m_used == -CUDART_INF_F) ? 0.f : ex2_approx(m_used - m_new)) : 1.f;
-          if (grow) { m_used = m_new; l_run *= f; }
-          if (it > 0) {  // S(it) complete => PV(it-1) complete (tensor pipe order): O may be rewritten
-#pragma unroll
-            for (int c = 0; c < D / 32; ++c) {
-              uint32_t v[32];
-              tmem_ld32(tO + lane_base + c * 32, v);
-              tmem_wait_ld();
-#pragma unroll
-              for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(__uint_as_float(v[i]) * f);
-              tmem_st32(tO + lane_base + c * 32, v);
+            for (int i = 0; i < 128; ++i) {
+              const int col = c0 + i;
+              if (!(col >= lo && col < hi)) sv[i] = 0xff800000u;  // -inf
             }
           }
-        }
-        const float neg_m = (m_used == -CUDART_INF_F) ? 0.f : -m_used;
-        // packed fp32 pairs (FFMA2 / FADD2): the two softmax warps of a scheduler are issue-bound, not MUFU-bound
-        const uint64_t sc2 = pack_f32x2(scale_log2, scale_log2), nm2 = pack_f32x2(neg_m, neg_m);
-        uint64_t ls2[4] = {0ull, 0ull, 0ull, 0ull};   // four pairs of partial row sums
+          float mx4[4] = {-CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F, -CUDART_INF_F};
 #pragma unroll
-        for (int half = 0; half < 2; ++half) {
+          for (int i = 0; i < 128; i += 4) {
 #pragma unroll
-          for (int c = half * 2; c < half * 2 + 2; ++c) {
-            uint32_t pk[16];
-#pragma unroll
-            for (int i = 0; i < 32; i += 2) {
-              float x0, x1;
-              unpack_f32x2(fma_f32x2(pack_f32x2(__uint_as_float(sv[c * 32 + i]), __uint_as_float(sv[c * 32 + i + 1])), sc2, nm2), x0, x1);
-              const float p0 = ex2_approx(x0), p1 = ex2_approx(x1);
-              ls2[(i >> 1) & 3] = add_f32x2(ls2[(i >> 1) & 3], pack_f32x2(p0, p1));
-              pk[i >> 1] = pack_bf16x2(p0, p1);
-            }
-            tmem_st16(tP + lane_base + c * 16, pk);
+            for (int e = 0; e < 4; ++e) mx4[e] = fmaxf(mx4[e], __uint_as_float(sv[i + e]));
           }
-          tmem_wait_st();
-          tc_fence_before();
-          mbar_arrive(bar_p + 8 * half);
-          if ((warp & 3) == 0 && lane == 0) FWD_STAMP(it, 17 + 8 * x + half);
-        }
-        {
-          float a0, a1;
-          unpack_f32x2(add_f32x2(add_f32x2(ls2[0], ls2[1]), add_f32x2(ls2[2], ls2[3])), a0, a1);
-          l_run += a0 + a1;
+          const float m_new = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * scale_log2;
+          // lazy rescale: only when the max moved by more than 2^8 (or the row saw its first key)
+          const bool grow = m_new > m_used + kRescaleThreshold || (m_used == -CUDART_INF_F && m_new > -CUDART_INF_F);
+          if (__any_sync(0xffffffffu, grow)) {
+            const float f = grow ? ((m_used == -CUDART_INF_F) ? 0.f : ex2_approx(m_used - m_new)) : 1.f;
+            if (grow) { m_used = m_new; l_run *= f; }
+            if (it > 0) {  // S(it) complete => PV(it-1) complete (tensor pipe order): O may be rewritten
+#pragma unroll
+              for (int c = 0; c < D / 32; ++c) {
+                uint32_t v[32];
+                tmem_ld32(tO + lane_base + c * 32, v);
+                tmem_wait_ld();
+#pragma unroll
+                for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(__uint_as_float(v[i]) * f);
+                tmem_st32(tO + lane_base + c * 32, v);
+              }
+            }
+          }
+          const float neg_m = (m_used == -CUDART_INF_F) ? 0.f : -m_used;
+          // packed fp32 pairs (FFMA2 / FADD2): the two softmax warps of a scheduler are issue-bound, not MUFU-bound
+          const uint64_t sc2 = pack_f32x2(scale_log2, scale_log2), nm2 = pack_f32x2(neg_m, neg_m);
+          uint64_t ls2[4] = {0ull, 0ull, 0ull, 0ull};   // four pairs of partial row sums
+#pragma unroll
+          for (int half = 0; half < 2; ++half) {
+#pragma unroll
+            for (int c = half * 2; c < half * 2 + 2; ++c) {
+              uint32_t pk[16];
+#pragma unroll
+              for (int i = 0; i < 32; i += 2) {
+                float x0, x1;
+                unpack_f32x2(fma_f32x2(pack_f32x2(__uint_as_float(sv[c * 32 + i]), __uint_as_float(sv[c * 32 + i + 1])), sc2, nm2), x0, x1);
+                const float p0 = ex2_approx(x0), p1 = ex2_approx(x1);
+                ls2[(i >> 1) & 3] = add_f32x2(ls2[(i >> 1) & 3], pack_f32x2(p0, p1));
+                pk[i >> 1] = pack_bf16x2(p0, p1);
+              }
+              tmem_st16(tP + lane_base + c * 16, pk);
+            }
+            tmem_wait_st();
+            tc_fence_before();
+            mbar_arrive_warp(bar_p + 8 * half);
+            if ((warp & 3) == 0 && lane == 0) FWD_STAMP(it, 17 + 8 * x + half);
+          }
+          {
+            float a0, a1;
+            unpack_f32x2(add_f32x2(add_f32x2(ls2[0], ls2[1]), add_f32x2(ls2[2], ls2[3])), a0, a1);
+            l_run += a0 + a1;
+          }
         }
       }
-    }
-    // ---- epilogue: O / l -> global, LSE (natural log)
-    if (n_iters > 0) {
-      mbar_wait(bar_o, 0);
-      tc_fence_after();
-    }
-    const float inv_l = l_run > 0.f ? 1.f / l_run : 0.f;
-    const size_t row_off = (static_cast<size_t>(t) * n_q_heads + h) * D;
-#pragma unroll
-    for (int c = 0; c < D / 32; ++c) {
-      uint32_t v[32];
+      // ---- epilogue: O / l -> global, LSE (natural log).  O leaves TMEM first and the columns are handed back, so the
+      // next item's first PV does not wait for the global stores.
+      const float inv_l = l_run > 0.f ? 1.f / l_run : 0.f;
+      const size_t row_off = (static_cast<size_t>(t) * n_q_heads + h) * D;
+      uint32_t o[D];
       if (n_iters > 0) {
-        tmem_ld32(tO + lane_base + c * 32, v);
+        mbar_wait(bar_o, nq & 1);
+        tc_fence_after();
+#pragma unroll
+        for (int c = 0; c < D / 32; ++c) tmem_ld32(tO + lane_base + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&o[c * 32]));
         tmem_wait_ld();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_oe);
+        ++nq;
       } else {
 #pragma unroll
-        for (int i = 0; i < 32; ++i) v[i] = 0u;
+        for (int i = 0; i < D; ++i) o[i] = 0u;
       }
       if (valid) {
         if (PARTIAL) {
-          float4* dst = reinterpret_cast<float4*>(out_f32 + row_off + c * 32);
+          float4* dst = reinterpret_cast<float4*>(out_f32 + row_off);
 #pragma unroll
-          for (int i = 0; i < 8; ++i)
-            dst[i] = make_float4(__uint_as_float(v[4 * i]) * inv_l, __uint_as_float(v[4 * i + 1]) * inv_l,
-                                 __uint_as_float(v[4 * i + 2]) * inv_l, __uint_as_float(v[4 * i + 3]) * inv_l);
+          for (int i = 0; i < D / 4; ++i)
+            dst[i] = make_float4(__uint_as_float(o[4 * i]) * inv_l, __uint_as_float(o[4 * i + 1]) * inv_l,
+                                 __uint_as_float(o[4 * i + 2]) * inv_l, __uint_as_float(o[4 * i + 3]) * inv_l);
         } else {
-          uint4* dst = reinterpret_cast<uint4*>(out + row_off + c * 32);
+          uint4* dst = reinterpret_cast<uint4*>(out + row_off);
 #pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            uint4 w;
-            w.x = pack_bf16x2(__uint_as_float(v[8 * i + 0]) * inv_l, __uint_as_float(v[8 * i + 1]) * inv_l);
-            w.y = pack_bf16x2(__uint_as_float(v[8 * i + 2]) * inv_l, __uint_as_float(v[8 * i + 3]) * inv_l);
-            w.z = pack_bf16x2(__uint_as_float(v[8 * i + 4]) * inv_l, __uint_as_float(v[8 * i + 5]) * inv_l);
-            w.w = pack_bf16x2(__uint_as_float(v[8 * i + 6]) * inv_l, __uint_as_float(v[8 * i + 7]) * inv_l);
-            dst[i] = w;
+          for (int i = 0; i < D / 8; ++i) {
+            uint4 wv;
+            wv.x = pack_bf16x2(__uint_as_float(o[8 * i + 0]) * inv_l, __uint_as_float(o[8 * i + 1]) * inv_l);
+            wv.y = pack_bf16x2(__uint_as_float(o[8 * i + 2]) * inv_l, __uint_as_float(o[8 * i + 3]) * inv_l);
+            wv.z = pack_bf16x2(__uint_as_float(o[8 * i + 4]) * inv_l, __uint_as_float(o[8 * i + 5]) * inv_l);
+            wv.w = pack_bf16x2(__uint_as_float(o[8 * i + 6]) * inv_l, __uint_as_float(o[8 * i + 7]) * inv_l);
+            dst[i] = wv;
           }
         }
+        lse[static_cast<size_t>(h) * n_tokens + t] = l_run > 0.f ? (m_used + log2f(l_run)) * kLn2 : -CUDART_INF_F;
       }
     }
-    if (valid)
-      lse[static_cast<size_t>(h) * n_tokens + t] = l_run > 0.f ? (m_used + log2f(l_run)) * kLn2 : -CUDART_INF_F;
   }
 
   tc_fence_before();
   __syncthreads();
   if (warp == 1) tmem_dealloc(tmem, 512);
+  if (threadIdx.x == 0) {   // the last CTA to leave re-arms the counters for the next launch
+    __threadfence();
+    if (atomicAdd(sched + 1, 1) == static_cast<int>(gridDim.x) - 1) { sched[0] = 0; sched[1] = 0; __threadfence(); }
+  }
 }
 
 }  // namespace sap

@@ -29,7 +29,7 @@ struct SegDesc {
 };
 
 struct TileProgram {
-  std::vector<TileDesc> tiles;  // longest first
+  std::vector<TileDesc> tiles;  // launch order: Q-stationary longest first; KV-stationary by document, longest first inside
   std::vector<SegDesc> segs;
   int64_t streamed_tiles = 0;   // total streamed 128x128 tiles (per head)
 };

@@ -83,6 +83,7 @@ void build_kv_program(const sap_plan& p, TileProgram& out, int32_t chunk_begin, 
   out.streamed_tiles = 0;
   const int64_t n = p.chunk_len, N = p.n_tokens;
   std::vector<int64_t> work;
+  std::vector<int32_t> group;
   // K/V tiles of `tile_rows` keys (128: one CTA; 256: a CTA pair) counted from the first key of the range (they must
   // match the key tiles the forward kernel streams only in coverage, not in alignment); a tile that straddles two
   // kv-chunks gets segments from both.
@@ -120,11 +121,24 @@ void build_kv_program(const sap_plan& p, TileProgram& out, int32_t chunk_begin, 
     if (drop_empty && td.seg_end == td.seg_begin) continue;
     out.tiles.push_back(td);
     work.push_back(w);
+    group.push_back(doc_of(p.cu, c1 - 1));
     out.streamed_tiles += w;
   }
+  // Order: tiles that stream the tail of the same document (the document of their last key) run side by side, so the
+  // rows they all add into - that document's part of the fp32 dQ accumulator, and its Q / dO rows - stay in L2 while
+  // they are live; documents longest first and, inside a document, longest tile first, so that the launch still ends on
+  // short tiles.
+  std::vector<int64_t> group_work(p.n_docs, 0);
+  for (size_t k = 0; k < work.size(); ++k) group_work[group[k]] = std::max(group_work[group[k]], work[k]);
   std::vector<int32_t> order(out.tiles.size());
   for (size_t k = 0; k < order.size(); ++k) order[k] = (int32_t)k;
-  std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return work[a] > work[b]; });
+  std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) {
+    if (group[a] != group[b]) {
+      if (group_work[group[a]] != group_work[group[b]]) return group_work[group[a]] > group_work[group[b]];
+      return group[a] < group[b];
+    }
+    return work[a] > work[b];
+  });
   std::vector<TileDesc> sorted(out.tiles.size());
   for (size_t k = 0; k < order.size(); ++k) sorted[k] = out.tiles[order[k]];
   out.tiles.swap(sorted);
