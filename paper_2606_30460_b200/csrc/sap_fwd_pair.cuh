@@ -33,7 +33,7 @@ struct FwdPairSmem {
   static constexpr int kOffK = 2 * kTileBytes;                      // K ring
   static constexpr int kOffV = kOffK + kFwdPairStages * kTileBytes; // V ring
   static constexpr int kBarOffset = kOffV + kFwdPairStages * kTileBytes;
-  static constexpr int kTotal = kBarOffset + 256;
+  static constexpr int kTotal = kBarOffset + 512;   // barriers [0,192) | TMEM slot 200 | work ring [256, 256 + 2 x 96)
 };
 
 // Work item w of a launch -> (kv-head, Q tile, first q-head of the pair): kv-head-major, tiles longest-first inside a
@@ -44,6 +44,21 @@ __device__ __forceinline__ FwdPairWork fwd_pair_work(int w, int n_tiles, int g) 
   const int hk = w / per_head, rem = w % per_head;
   return {hk, rem / pairs, hk * g + 2 * (rem % pairs)};
 }
+// One slot of the work ring the scheduler thread fills ahead of the other roles: everything they need to start an item
+// without a global load of their own (tile, first segment, iteration count, and the cu_seqlens entries around the tile's
+// first row, from which each row finds the start of its document).
+constexpr int kFwdCuWindow = 8;
+struct FwdWorkSlot {
+  int32_t w;            // work item, -1 = no more work
+  int32_t row0, rows, seg_begin, seg_end;
+  int32_t n_iters;      // streamed K/V tiles of the item
+  int32_t n_cu;         // valid entries of cu_win
+  int32_t pad;
+  int32_t cu_win[kFwdCuWindow];   // cu[e0 .. e0 + n_cu), e0 = document of row0
+  SegDesc seg0;         // segs[seg_begin] (valid if n_iters > 0)
+};
+static_assert(sizeof(FwdWorkSlot) == 96, "work ring slot layout");
+
 __device__ __forceinline__ int fwd_tile_iters(const TileDesc& td, const SegDesc* __restrict__ segs) {
   int n = 0;
   for (int s = td.seg_begin; s < td.seg_end; ++s) n += (segs[s].t_end - segs[s].t_begin + kTile - 1) / kTile;
@@ -67,8 +82,8 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
   const uint32_t s0 = smem_u32(smem);
   const uint32_t sQ = s0 + L::kOffQ, sK = s0 + L::kOffK, sV = s0 + L::kOffV;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L::kBarOffset);
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kBarOffset + 240);
-  volatile int* work_ring = reinterpret_cast<volatile int*>(smem + L::kBarOffset + 224);   // 2 slots
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kBarOffset + 200);
+  volatile FwdWorkSlot* work_ring = reinterpret_cast<volatile FwdWorkSlot*>(smem + L::kBarOffset + 256);   // 2 slots
   const uint32_t bar_q_full = smem_u32(bars + 0), bar_k_full = smem_u32(bars + 1), bar_k_empty = smem_u32(bars + 3),
                  bar_v_full = smem_u32(bars + 5), bar_v_empty = smem_u32(bars + 7),
                  bar_s_full = smem_u32(bars + 9) /* [A, B] */, bar_p_full = smem_u32(bars + 11) /* [A0, A1, B0, B1] */,
@@ -109,14 +124,35 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
         int ws = 0, wph = 1, nq = 0;   // work ring slot / phase; items with loads so far
         for (int w = blockIdx.x;; w = gridDim.x + atomicAdd(sched, 1)) {
           const bool end = w >= n_work;
+          FwdPairWork wk = {0, 0, 0};
+          TileDesc td = {0, 0, 0, 0};
+          int n_it = 0, e0 = 0, n_cu = 0;
+          if (!end) {   // all global loads of the item's metadata happen here, ahead of the roles that use it
+            wk = fwd_pair_work(w, n_tiles, g);
+            td = tiles[wk.tile_idx];
+            n_it = fwd_tile_iters(td, segs);
+            int lo = 0, hi = n_docs;   // e0 = document of row0: cu[e0] <= row0 < cu[hi]
+            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (__ldg(cu + mid) <= td.row0) lo = mid; else hi = mid; }
+            e0 = lo;
+            n_cu = min(kFwdCuWindow, n_docs + 1 - e0);
+          }
           mbar_wait(bar_w_empty + 8 * ws, wph);
-          work_ring[ws] = end ? -1 : w;
+          volatile FwdWorkSlot* slot = work_ring + ws;
+          slot->w = end ? -1 : w;
+          if (!end) {
+            slot->row0 = td.row0; slot->rows = td.rows; slot->seg_begin = td.seg_begin; slot->seg_end = td.seg_end;
+            slot->n_iters = n_it; slot->n_cu = n_cu;
+            for (int j = 0; j < n_cu; ++j) slot->cu_win[j] = __ldg(cu + e0 + j);
+            if (n_it > 0) {
+              const SegDesc sd = segs[td.seg_begin];
+              slot->seg0.t_begin = sd.t_begin; slot->seg0.t_end = sd.t_end; slot->seg0.q_lo = sd.q_lo; slot->seg0.q_hi = sd.q_hi;
+              slot->seg0.kv_lo = sd.kv_lo; slot->seg0.kv_hi = sd.kv_hi; slot->seg0.item = sd.item;
+            }
+          }
           mbar_arrive(bar_w_full + 8 * ws);   // release: the slot is written
           if (++ws == 2) { ws = 0; wph ^= 1; }
           if (end) break;
-          const FwdPairWork wk = fwd_pair_work(w, n_tiles, g);
-          const TileDesc td = tiles[wk.tile_idx];
-          if (fwd_tile_iters(td, segs) == 0) continue;
+          if (n_it == 0) continue;
           mbar_wait(bar_q_empty, (nq & 1) ^ 1);   // the last S of the previous item has read Q
           ++nq;
           mbar_expect_tx(bar_q_full, 2 * L::kTileBytes);
@@ -163,12 +199,10 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
         int ws = 0, wph = 0;
         for (;;) {
           mbar_wait(bar_w_full + 8 * ws, wph);
-          const int w = work_ring[ws];
+          const int w = work_ring[ws].w, n_iters = work_ring[ws].n_iters;
           mbar_arrive(bar_w_empty + 8 * ws);
           if (++ws == 2) { ws = 0; wph ^= 1; }
           if (w < 0) break;
-          const FwdPairWork wk = fwd_pair_work(w, n_tiles, g);
-          const int n_iters = fwd_tile_iters(tiles[wk.tile_idx], segs);
           if (n_iters == 0) continue;
           auto issue_pv = [&](int x, int st_, int it) {  // O_x += P_x V, in two halves of 64 keys
 #pragma unroll
@@ -235,26 +269,48 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     int gi = 0, nq = 0, ws = 0, wph = 0;
     for (;;) {
       mbar_wait(bar_w_full + 8 * ws, wph);
-      const int w = work_ring[ws];
+      volatile FwdWorkSlot* slot = work_ring + ws;
+      const int w = slot->w;
+      TileDesc td = {0, 0, 0, 0};
+      SegDesc sd = {0, 0, 0, 0, 0, 0, 0, 0};
+      int n_iters = 0, t = 0;
+      int32_t doc_lo = 0;
+      bool valid = false, far = false;
+      if (w >= 0) {
+        td.row0 = slot->row0; td.rows = slot->rows; td.seg_begin = slot->seg_begin; td.seg_end = slot->seg_end;
+        n_iters = slot->n_iters;
+        t = td.row0 + r;
+        valid = r < td.rows;
+        const int n_cu = slot->n_cu;
+        doc_lo = slot->cu_win[0];   // start of the row's document: the last window entry <= t (cu is non-decreasing)
+#pragma unroll
+        for (int j = 1; j < kFwdCuWindow; ++j) {
+          const int32_t c = slot->cu_win[j];
+          if (j < n_cu && c <= t) doc_lo = c;
+        }
+        far = valid && n_cu == kFwdCuWindow && slot->cu_win[kFwdCuWindow - 1] <= t;   // more than 7 documents start inside the tile before this row
+        if (n_iters > 0) {
+          sd.t_begin = slot->seg0.t_begin; sd.t_end = slot->seg0.t_end; sd.q_lo = slot->seg0.q_lo; sd.q_hi = slot->seg0.q_hi;
+          sd.kv_lo = slot->seg0.kv_lo; sd.kv_hi = slot->seg0.kv_hi;
+        }
+      }
       __syncwarp();
       if (lane == 0) mbar_arrive(bar_w_empty + 8 * ws);
       if (++ws == 2) { ws = 0; wph ^= 1; }
       if (w < 0) break;
+      if (far) doc_lo = doc_start_of(cu, n_docs, t);
       const FwdPairWork wk = fwd_pair_work(w, n_tiles, g);
-      const TileDesc td = tiles[wk.tile_idx];
-      const int n_iters = fwd_tile_iters(td, segs);
       const int h = wk.h0 + x;
-      const int t = td.row0 + r;
-      const bool valid = r < td.rows;
-      const int32_t doc_lo = valid ? doc_start_of(cu, n_docs, t) : 0;
       float m_used = -CUDART_INF_F;  // reference max (log2 domain) the running sum and O are scaled by
       float l_run = 0.f;
       int it = 0;
       for (int s = td.seg_begin; s < td.seg_end; ++s) {
-        const SegDesc sd = segs[s];
+        // the next segment's descriptor is loaded one segment ahead (its latency hides behind this segment's tiles)
+        const SegDesc sd_next = segs[s + 1 < td.seg_end ? s + 1 : s];
         int lo = max(doc_lo, sd.kv_lo), hi = min(t + 1, sd.kv_hi);  // visible keys of this row: [lo, hi)
         if (!valid || t < sd.q_lo || t >= sd.q_hi) { lo = 0; hi = 0; }
-        for (int c0 = sd.t_begin; c0 < sd.t_end; c0 += kTile, ++it, ++gi) {
+        const int c_end = sd.t_end;
+        for (int c0 = sd.t_begin; c0 < c_end; c0 += kTile, ++it, ++gi) {
           mbar_wait(bar_s, gi & 1);
           tc_fence_after();
           if ((warp & 3) == 0 && lane == 0) FWD_STAMP(it, 16 + 8 * x);
@@ -324,6 +380,7 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
             l_run += a0 + a1;
           }
         }
+        sd = sd_next;
       }
       // ---- epilogue: O / l -> global, LSE (natural log).  O leaves TMEM first and the columns are handed back, so the
       // next item's first PV does not wait for the global stores.
