@@ -421,6 +421,9 @@ def run_ours(args):
         else:
             # main kernel: all 5 GEMMs of the backward (the D pre-pass line includes zeroing the fp32 dQ accumulator)
             kernels[main_kernel] = {"ms": per["bwd_fused"], "algorithmic_tflop": 5 * gemm / 1e12}
+            # sap_attn_bwd_begin = D pre-pass + cudaMemsetAsync of the fp32 dQ accumulator: count the zeroed bytes too
+            kernels["sap_bwd_pre_kernel"]["algorithmic_gbytes"] += N * Hq * d * 4 / 1e9
+            kernels["sap_bwd_pre_kernel"]["includes"] = "cudaMemsetAsync of the fp32 dQ accumulator"
             kernels["sap_bwd_post_kernel"] = {"ms": per["bwd_post"], "algorithmic_gbytes": N * Hq * d * 6 / 1e9}
         for kk, vv in kernels.items():
             if "algorithmic_tflop" in vv:
