@@ -184,6 +184,38 @@ def table2_context(dev, steps: int = 5):
     return res
 
 
+def d64_context(dev, steps: int = 3):
+    """SURVEY 8(f) NEXT-4, head_dim 64: configs[2]'s packing with 64 q-heads / 16 kv-heads of 64 (the same bytes per token),
+    forward and backward timed apart.  At d = 64 a score costs half the tensor work but the same exponential: the
+    forward keeps the MUFU (16 exp / clk / SM) over 80 % busy and cannot reach the d = 128 rate."""
+    import torch
+    import paper_2606_30460_b200 as sap
+    from paper_2606_30460_b200.workloads import custom_workload, make_qkv, make_workload
+    w0 = make_workload(3)
+    w = custom_workload(w0.doc_lens, w0.n_chunks, 64, 16, 64, name="configs[2] packing, 64/16 heads, d=64")
+    q, k, v, do = make_qkv(w, device=dev)
+    plan = sap.sap_plan(w.cu_seqlens, w.n_chunks); plan.upload()
+    cu = plan.cu_seqlens_dev(dev)
+    out = torch.empty_like(q); lse = torch.empty((w.n_q_heads, w.n_tokens), dtype=torch.float32, device=dev)
+    dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(v)
+    ws = torch.empty(sap.sap_workspace_bytes(plan, w.n_q_heads, w.n_kv_heads, w.head_dim, sap.SAP_PASS_BWD), dtype=torch.uint8, device=dev)
+    fns = {"fwd": lambda: sap.sap_attn_fwd(q, k, v, cu, plan, out, lse, softmax_scale=w.softmax_scale),
+           "bwd": lambda: sap.sap_attn_bwd(do, q, k, v, out, lse, cu, plan, softmax_scale=w.softmax_scale, dq=dq, dk=dk, dv=dv, workspace=ws)}
+    res = {"workload": w.name}
+    for name, fn in fns.items():
+        for _ in range(3):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); e0.record()
+        for _ in range(steps):
+            fn()
+        e1.record(); torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        fl = w.flops_fwd if name == "fwd" else w.flops_bwd
+        res[name] = {"ms": ms, "tflops": fl / (ms * 1e-3) / 1e12}
+    return res
+
+
 def kernel_source_sha256():
     """Hash of every source file that goes into libsap_b200.so: the key of profiles/traffic.json."""
     import hashlib
@@ -443,6 +475,7 @@ def run_ours(args):
                     "ms_per_launch": kernels[dom]["ms"],
                     "traffic_source": traffic_src}
         t2 = table2_context(dev) if (world == 1 and args.config == 3) else None
+        d64 = d64_context(dev) if (world == 1 and args.config == 3) else None
         cdt, cfl, cthreads, cdesc = time_oracle_sample()
         c1dt, c1fl, _, c1desc = time_oracle_cfg1()
         line = {
@@ -474,7 +507,7 @@ def run_ours(args):
             "cpu_baseline": {"value": cfl / cdt / 1e12, "unit": UNIT, "cores": cthreads, "kind": "oracle",
                              "sample": cdesc, "seconds": cdt,
                              "cfg1_full": {"value": c1fl / c1dt / 1e12, "unit": UNIT, "seconds": c1dt, "sample": c1desc}},
-            "table2_context": t2,
+            "table2_context": t2, "d64_context": d64,
             "paper_context": "HSAP Table 2 (PAPER.md:158-164): SAP attention fwd+bwd 128K/SP16 = 3333.1 ms on A100s, "
                              "multi-GPU, communication included; not comparable, context only",
         }
