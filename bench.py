@@ -391,10 +391,11 @@ def run_ours(args):
     s_comp, s_h2d, s_d2h = torch.cuda.current_stream(), torch.cuda.Stream(), torch.cuda.Stream()
     d_in = [(q, k, v, do), tuple(torch.empty_like(x) for x in (q, k, v, do))]
     d_out = [(out, lse, dq, dk, dv), tuple(torch.empty_like(x) for x in (out, lse, dq, dk, dv))]
-    h_in, h_out = (hq, hk, hv, hdo), (r_out, r_lse, r_dq, r_dk, r_dv)
 
     def e2e_run(n):
-        in_ready = [torch.cuda.Event() for _ in range(n)]
+        qkv_ready = [torch.cuda.Event() for _ in range(n)]
+        do_ready = [torch.cuda.Event() for _ in range(n)]
+        fwd_done = [torch.cuda.Event() for _ in range(n)]
         comp_done = [torch.cuda.Event() for _ in range(n)]
         d2h_done = [torch.cuda.Event() for _ in range(n)]
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -402,24 +403,30 @@ def run_ours(args):
         e0.record(s_h2d)
         for i in range(n):
             sl = i & 1
+            qi, ki, vi, doi = d_in[sl]
+            oi, li, dqi, dki, dvi = d_out[sl]
             with torch.cuda.stream(s_h2d):
                 if i >= 2:
                     s_h2d.wait_event(comp_done[i - 2])          # the slot's inputs have been consumed
-                for dst, src in zip(d_in[sl], h_in):
+                for dst, src in zip((qi, ki, vi), (hq, hk, hv)):
                     dst.copy_(src, non_blocking=True)
-                in_ready[i].record(s_h2d)
-            s_comp.wait_event(in_ready[i])
+                qkv_ready[i].record(s_h2d)                      # the forward needs only Q, K, V ...
+                doi.copy_(hdo, non_blocking=True)
+                do_ready[i].record(s_h2d)                       # ... dO travels under it
+            s_comp.wait_event(qkv_ready[i])
             if i >= 2:
                 s_comp.wait_event(d2h_done[i - 2])              # the slot's previous results have been read back
-            qi, ki, vi, doi = d_in[sl]
-            oi, li, dqi, dki, dvi = d_out[sl]
             sap.sap_attn_fwd(qi, ki, vi, cu, plan, oi, li, softmax_scale=w.softmax_scale)
+            fwd_done[i].record(s_comp)
+            s_comp.wait_event(do_ready[i])
             sap.sap_attn_bwd(doi, qi, ki, vi, oi, li, cu, plan, softmax_scale=w.softmax_scale, dq=dqi, dk=dki, dv=dvi,
                              workspace=ws)
             comp_done[i].record(s_comp)
             with torch.cuda.stream(s_d2h):
+                s_d2h.wait_event(fwd_done[i])                   # out and LSE go back while the backward runs
+                r_out.copy_(oi, non_blocking=True); r_lse.copy_(li, non_blocking=True)
                 s_d2h.wait_event(comp_done[i])
-                for dst, src in zip(h_out, d_out[sl]):
+                for dst, src in zip((r_dq, r_dk, r_dv), (dqi, dki, dvi)):
                     dst.copy_(src, non_blocking=True)
                 d2h_done[i].record(s_d2h)
         e1.record(s_d2h)
@@ -500,7 +507,7 @@ def run_ours(args):
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": ms_e2e_max, "steps": e_steps,
-                    "pipeline": "double-buffered, 3 streams: H2D of step i+1 and D2H of step i-1 overlap step i"},
+                    "pipeline": "double-buffered, 3 streams: H2D of step i+1 and D2H of step i-1 overlap step i; dO travels under the forward, out / LSE go back under the backward"},
             "gpu_launches": int(launches),
             "roofline": roofline,
             "kernels": kernels,
