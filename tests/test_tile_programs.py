@@ -90,3 +90,44 @@ def test_pair_tiles_are_256_keys_from_the_range_start():
     assert sorted(t[0] for t in tiles.tolist()) == list(range(0, 2048, 256)) and all(t[1] == 256 for t in tiles.tolist())
     tiles, _ = plan.tile_program(7, 1, 3)                         # kv-chunks 1..2: rows 512..1535
     assert sorted(t[0] for t in tiles.tolist()) == [512, 768, 1024, 1280]
+
+
+def _work(tiles, segs, tile_rows=128):
+    return [sum((te - tb + 127) // 128 for tb, te, *_ in segs[sb:se].tolist()) for _, _, sb, se in tiles.tolist()]
+
+
+@pytest.mark.parametrize("kind", [1, 2])
+def test_kv_tiles_are_launched_document_by_document(kind):
+    """Launch order of the KV-stationary programs: the tiles whose last key lies in one document
+    are adjacent, documents in order of their longest tile, and inside a document longest tile first - so the rows the
+    concurrently running tiles add into (that document's part of the dQ accumulator) stay in L2."""
+    cu = [0, 300, 300, 2900, 3000, 7000, 7100, 8192]
+    plan = sap.sap_plan(cu, 8)
+    tiles, segs = plan.tile_program(kind)
+    work = _work(tiles, segs)
+    doc = [int(np.searchsorted(np.asarray(cu), r0 + rows - 1, side="right") - 1) for r0, rows, _, _ in tiles.tolist()]
+    seen, prev = [], None
+    for d in doc:                                                # contiguous groups
+        if d != prev:
+            assert d not in seen, (doc, "tiles of one document are not adjacent")
+            seen.append(d); prev = d
+    best = {d: max(w for w, dd in zip(work, doc) if dd == d) for d in seen}
+    assert [best[d] for d in seen] == sorted((best[d] for d in seen), reverse=True)      # documents: longest tile first
+    for d in seen:
+        w = [x for x, dd in zip(work, doc) if dd == d]
+        assert w == sorted(w, reverse=True)                      # inside a document: longest first
+
+
+def test_q_tiles_are_longest_first_below_the_grouping_threshold():
+    """The Q-stationary program of a sequence below 192K tokens is plain longest-first (sap_plan.cpp:
+    kGroupQTilesFromTokens); from there on its tiles are grouped by the document of their first row."""
+    plan = sap.sap_plan([0, 300, 2900, 3000, 7000, 8192], 8)
+    tiles, segs = plan.tile_program(0)
+    work = _work(tiles, segs)
+    assert work == sorted(work, reverse=True)
+    big = [0, 100_000, 150_000, 196_608]                        # 192K tokens: grouped
+    plan = sap.sap_plan(big, 8)
+    tiles, segs = plan.tile_program(0)
+    doc = [int(np.searchsorted(np.asarray(big), r0, side="right") - 1) for r0, _, _, _ in tiles.tolist()]
+    changes = sum(1 for a, b in zip(doc, doc[1:]) if a != b)
+    assert changes == 2 and doc[0] == 0                          # three groups, the 100K-token document first
