@@ -264,6 +264,27 @@ int sap_axpy(void* dst, int dst_is_bf16, const void* src, int src_is_bf16, int64
              void* cuda_stream);
 
 /* ---- diagnostics ---------------------------------------------------------------------------- */
+/* ---- stitched allocation: the data plane of real ranks ------------------------------ */
+/* One device virtual address range of n_chunks * chunk_bytes bytes whose chunk c is physical memory of device
+ * device_of_chunk[c], readable and writable by every device in access_devices - the layout that lets a rank's launch
+ * (sap_attn_fwd_chunks, sap_attn_bwd_chunks) read the K/V shards its plan names where they live and add its dQ
+ * contributions into their owner's accumulator, instead of the grouped send / recv of PAPER.md:59, :100-102, :124 (inside
+ * an NVLink / NVSwitch domain).  A tensor [N, H, d] placed at sap_stitched_ptr has rows [c n, (c+1) n) of chunk c in
+ * device_of_chunk[c]'s memory when chunk_bytes = n * H * d * sizeof(element).
+ * chunk_bytes must be a multiple of sap_stitched_granularity of every owner (2 MiB on B200), else SAP_ERR_UNSUPPORTED.
+ * All arrays are host arrays, read.  Synchronous (CUDA virtual-memory API); several devices need P2P access between them
+ * (SAP_ERR_CUDA with the CUresult in sap_last_cuda_error otherwise).  The range belongs to the handle: sap_stitched_free
+ * unmaps and releases it (NULL is a no-op); the caller must have finished all work that uses it.
+ * One process driving several devices; handles are not exported to other processes. */
+typedef struct sap_stitched sap_stitched_t;
+int sap_stitched_granularity(int device, size_t* bytes);
+int sap_stitched_alloc(int32_t n_chunks, size_t chunk_bytes, const int32_t* device_of_chunk, int32_t n_access,
+                       const int32_t* access_devices, sap_stitched_t** out);
+void* sap_stitched_ptr(const sap_stitched_t* s);            /* device pointer of the range (NULL for NULL) */
+size_t sap_stitched_bytes(const sap_stitched_t* s);         /* n_chunks * chunk_bytes */
+int32_t sap_stitched_owner(const sap_stitched_t* s, int32_t chunk);   /* device that holds chunk, -1 if out of range */
+void sap_stitched_free(sap_stitched_t* s);
+
 const char* sap_strerror(int status);
 int sap_last_cuda_error(void);      /* the cudaError_t / CUresult of the last SAP_ERR_CUDA on this thread */
 /* Number of kernels the library has launched in this process (all streams); for launch accounting. */

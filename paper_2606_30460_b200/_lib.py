@@ -58,6 +58,12 @@ SIGNATURES = {
     "sap_axpy": (ctypes.c_int, [vp, ctypes.c_int, vp, ctypes.c_int, ctypes.c_int64, ctypes.c_float, ctypes.c_int, vp]),
     "sap_attn_bwd_end": (ctypes.c_int, [vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                         ctypes.c_float, vp, ctypes.c_size_t, vp]),
+    "sap_stitched_granularity": (ctypes.c_int, [ctypes.c_int, ctypes.POINTER(ctypes.c_size_t)]),
+    "sap_stitched_alloc": (ctypes.c_int, [ctypes.c_int32, ctypes.c_size_t, c_i32p, ctypes.c_int32, c_i32p, ctypes.POINTER(vp)]),
+    "sap_stitched_ptr": (vp, [vp]),
+    "sap_stitched_bytes": (ctypes.c_size_t, [vp]),
+    "sap_stitched_owner": (ctypes.c_int32, [vp, ctypes.c_int32]),
+    "sap_stitched_free": (None, [vp]),
     "sap_strerror": (ctypes.c_char_p, [ctypes.c_int]),
     "sap_last_cuda_error": (ctypes.c_int, []),
     "sap_launch_count": (ctypes.c_int64, []),

@@ -332,3 +332,61 @@ def sap_axpy(dst, src, alpha: float = 1.0, accumulate: bool = True, stream=None)
     _check(_lib.lib().sap_axpy(_ptr(dst), int(dst.dtype == torch.bfloat16), _ptr(src), int(src.dtype == torch.bfloat16),
                                dst.numel(), float(alpha), int(accumulate), _stream(stream)), "sap_axpy")
     return dst
+
+
+class Stitched:
+    """sap_stitched_alloc: one device address range of n_chunks * chunk_bytes bytes whose chunk c is memory of device
+    devices[c] (SURVEY 8(f) NEXT-1 data plane).  `tensor(shape, dtype)` views the range as a torch tensor (the range
+    stays alive as long as this object does: keep it)."""
+
+    def __init__(self, n_chunks: int, chunk_bytes: int, devices: Optional[Sequence[int]] = None,
+                 access_devices: Optional[Sequence[int]] = None):
+        devices = [0] * n_chunks if devices is None else [int(d) for d in devices]
+        access = sorted(set(devices)) if access_devices is None else [int(d) for d in access_devices]
+        self.handle = ctypes.c_void_p()
+        dev = (ctypes.c_int32 * len(devices))(*devices)
+        acc = (ctypes.c_int32 * len(access))(*access)
+        _check(_lib.lib().sap_stitched_alloc(int(n_chunks), int(chunk_bytes), dev, len(access), acc,
+                                             ctypes.byref(self.handle)), "sap_stitched_alloc")
+        self.ptr = int(_lib.lib().sap_stitched_ptr(self.handle))
+        self.nbytes = int(_lib.lib().sap_stitched_bytes(self.handle))
+        self.n_chunks, self.chunk_bytes, self.devices = int(n_chunks), int(chunk_bytes), devices
+
+    @staticmethod
+    def granularity(device: int = 0) -> int:
+        g = ctypes.c_size_t()
+        _check(_lib.lib().sap_stitched_granularity(int(device), ctypes.byref(g)), "sap_stitched_granularity")
+        return int(g.value)
+
+    def owner(self, chunk: int) -> int:
+        return int(_lib.lib().sap_stitched_owner(self.handle, int(chunk)))
+
+    def tensor(self, shape, dtype, device=None):
+        import torch
+        nbytes = int(np.prod(shape)) * torch.empty((), dtype=dtype).element_size()
+        if nbytes > self.nbytes:
+            raise ValueError(f"shape {tuple(shape)} needs {nbytes} bytes, the range has {self.nbytes}")
+        typestr = {torch.bfloat16: "<u2", torch.float32: "<f4", torch.uint8: "|u1", torch.int32: "<i4"}[dtype]
+
+        class _View:   # __cuda_array_interface__: torch wraps the memory, it does not own it
+            __cuda_array_interface__ = {"shape": (nbytes // int(typestr[2]),), "typestr": typestr, "data": (self.ptr, False),
+                                        "version": 2}
+        t = torch.as_tensor(_View(), device=device if device is not None else f"cuda:{self.devices[0]}")
+        if dtype == torch.bfloat16:
+            t = t.view(torch.bfloat16)
+        t = t.view(*shape)
+        t._sap_stitched = self   # the tensor keeps the range alive
+        return t
+
+    def free(self):
+        if getattr(self, "handle", None) is not None and self.handle:
+            import torch
+            torch.cuda.synchronize()   # no kernel may still be using the range when it is unmapped
+            _lib.lib().sap_stitched_free(self.handle)
+            self.handle = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
