@@ -258,18 +258,123 @@ def run_dry(args):
     rank, world, _ = shard.rank_world()
     if world > 1:
         dist.init_process_group("gloo")
-    w, heads = shard.rank_share(args.config, rank, world, args.shard)
+    extra = {}
+    if args.shard == "chunks":       # one sequence, every head, rank r launches the chunks ranks.launch_chunks gives it
+        from paper_2606_30460_b200.ranks import launch_chunks
+        w = shard.rank_workload(args.config, 0)
+        heads, share = tuple(range(w.n_kv_heads)), 1.0 / world
+        extra = {"chunks_launched_by_rank": [launch_chunks(r, world, w.n_chunks) for r in range(world)]}
+    else:
+        w, heads = shard.rank_share(args.config, rank, world, args.shard)
+        share = len(heads) / w.n_kv_heads
     plan = sap.sap_plan(w.cu_seqlens, w.n_chunks)
-    share = len(heads) / w.n_kv_heads
     ms_max, flops_all = shard.aggregate(1.0 + rank, float(w.flops_fwd + w.flops_bwd) * share)
     if rank == 0:
-        print(json.dumps({"dry_run": True, "metric": METRIC, "n_gpus": world, "shard": args.shard,
-                          "scaling": "strong" if args.shard == "heads" else "weak", "plan_items": plan.n_items,
+        print(json.dumps({"dry_run": True, "metric": METRIC, "n_gpus": world, "shard": args.shard, **extra,
+                          "scaling": "weak" if args.shard == "seqs" else "strong", "plan_items": plan.n_items,
                           "kv_heads_of_rank0": list(heads), "whole_job_tflop_per_step": flops_all / 1e12,
                           "max_over_ranks_check": ms_max == float(world),
                           "config": {"workload": w.name, "n_tokens": w.n_tokens}}), flush=True)
     if world > 1:
         dist.barrier()
+        dist.destroy_process_group()
+
+
+def run_chunks(args):
+    """`--shard chunks`: the paper's sequence parallelism itself.  ONE packed sequence; rank r owns the
+    memory of a contiguous block of its chunks (stitched tensors: ranks.ProcessRank) and launches the library's kernels on
+    the chunks the zig-zag assignment gives it; K/V, Q/dO and the dQ contributions travel inside the kernels (TMA and
+    red.global over NVLink), the only synchronisation is four group barriers per step.  Strong scaling.  A step also
+    includes, under `e2e`, every rank's own rows going host -> device and its results coming back."""
+    import torch
+    import torch.distributed as dist
+    import paper_2606_30460_b200 as sap
+    from paper_2606_30460_b200 import shard
+    from paper_2606_30460_b200.ranks import ProcessRank
+    from paper_2606_30460_b200.workloads import make_qkv
+
+    rank, world, local = shard.rank_world()
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    w = shard.rank_workload(args.config, 0)                     # the same sequence on every rank
+    if w.n_chunks % world != 0:
+        raise ValueError(f"--shard chunks needs n_chunks ({w.n_chunks}) divisible by the number of ranks ({world})")
+    N, Hq, Hkv, d = w.n_tokens, w.n_q_heads, w.n_kv_heads, w.head_dim
+    pr = ProcessRank(w.cu_seqlens, rank, world, device=local, n_chunks=w.n_chunks)
+    q, do, out, dq = (pr.tensor((Hq, d), torch.bfloat16) for _ in range(4))
+    k, v, dk, dv = (pr.tensor((Hkv, d), torch.bfloat16) for _ in range(4))
+    lse = pr.shared((Hq, N), torch.float32)
+    ws = pr.workspace(Hq, Hkv, d)
+    rows = pr.own_rows()
+    src = make_qkv(w, device=dev)                               # seeded: every rank can generate it, keeps its own rows
+    host_in = [t[rows].cpu().pin_memory() for t in src]
+    for dst, t in zip((q, k, v, do), src):
+        dst[rows].copy_(t[rows])
+    del src
+    host_out = [torch.empty_like(t[rows], device="cpu").pin_memory() for t in (out, dq, dk, dv)]
+    pr.barrier()
+
+    def step():
+        pr.forward(q, k, v, out, lse, softmax_scale=w.softmax_scale)
+        pr.backward(do, q, k, v, out, lse, dq, dk, dv, ws, softmax_scale=w.softmax_scale)
+
+    def step_e2e():
+        for dst, t in zip((q, k, v, do), host_in):
+            dst[rows].copy_(t, non_blocking=True)
+        pr.barrier()                                            # everybody's inputs of this step are in place
+        step()
+        for dst, t in zip(host_out, (out, dq, dk, dv)):
+            dst.copy_(t[rows], non_blocking=True)
+        torch.cuda.synchronize()
+
+    def timed(fn, n):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        pr.barrier()
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = sap.sap_launch_count()
+    ms = timed(step, args.steps)
+    launches = sap.sap_launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    flops = float(w.flops_fwd + w.flops_bwd)
+    ms_max, flops_all = shard.aggregate(ms, flops / world, dev)
+    ms_e2e = timed(step_e2e, max(3, min(args.steps, 10)))
+    ms_e2e_max, _ = shard.aggregate(ms_e2e, 0.0, dev)
+    if rank == 0:
+        peaks = load_peaks()
+        value = flops_all / (ms_max * 1e-3) / 1e12
+        h2d = sum(t.numel() * t.element_size() for t in host_in) * world
+        d2h = sum(t.numel() * t.element_size() for t in host_out) * world
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_max, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic",
+            "config": {"workload": w.name, "n_tokens": N, "n_docs": len(w.doc_lens), "n_chunks": w.n_chunks, "n_q_heads": Hq,
+                       "n_kv_heads": Hkv, "head_dim": d, "cu_seqlens_sha256": w.sha256(), "shard": "chunks",
+                       "per_rank": "one sequence; rank r owns the memory of chunks %s.. and launches %s (zig-zag); stitched tensors, "
+                                   "4 group barriers per step, no collective on the data path" % (pr.owned[0], pr.launch),
+                       "l2": "inputs exceed L2"},
+            "frac_of_bf16_peak": {"measured_burst": value / world / peaks["bf16_burst"],
+                                  "measured_sustained": value / world / peaks["bf16_sustained"], "source": peaks["source"]},
+            "clocks": clocks, "gpu_launches": launches * world,
+            "e2e": {"value": flops_all / (ms_e2e_max * 1e-3) / 1e12, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e_max,
+                    "pipeline": "every rank copies its own rows in and its own results out, not overlapped"},
+            "roofline": None, "cpu_baseline": None}), flush=True)
+    pr.barrier()
+    if world > 1:
         dist.destroy_process_group()
 
 
@@ -535,8 +640,9 @@ def main():
                     help="forward kernel: two q-heads per CTA (default when Hq/Hkv is even) or one (diagnostic)")
     ap.add_argument("--bwd", default="fused", choices=["fused", "split"],
                     help="backward form: fused 5-GEMM kernel (default) or the split dK/dV + dQ kernels (diagnostic)")
-    ap.add_argument("--shard", default="seqs", choices=["seqs", "heads"],
-                    help="multi-GPU split: independent sequences per rank (weak scaling) or the kv-heads of one sequence (strong)")
+    ap.add_argument("--shard", default="seqs", choices=["seqs", "heads", "chunks"],
+                    help="multi-GPU split: independent sequences per rank (weak scaling), the kv-heads of one sequence (strong), or "
+                         "the chunks of one sequence = the paper's sequence parallelism over stitched tensors (strong)")
     ap.add_argument("--dry-run", action="store_true", help="host side only (planner, sharding, aggregation over gloo); no GPU")
     ap.add_argument("--profile-only", action="store_true",
                     help="stop after the device-timed region and the per-kernel passes (for ncu runs)")
@@ -547,6 +653,8 @@ def main():
         run_reference(args)
     elif args.dry_run:
         run_dry(args)
+    elif args.shard == "chunks":
+        run_chunks(args)
     else:
         run_ours(args)
 

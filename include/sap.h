@@ -275,7 +275,8 @@ int sap_axpy(void* dst, int dst_is_bf16, const void* src, int src_is_bf16, int64
  * All arrays are host arrays, read.  Synchronous (CUDA virtual-memory API); several devices need P2P access between them
  * (SAP_ERR_CUDA with the CUresult in sap_last_cuda_error otherwise).  The range belongs to the handle: sap_stitched_free
  * unmaps and releases it (NULL is a no-op); the caller must have finished all work that uses it.
- * One process driving several devices; handles are not exported to other processes. */
+ * This call is the form for one process driving several devices; sap_stitched_create_local below is the one for one
+ * process per GPU. */
 typedef struct sap_stitched sap_stitched_t;
 int sap_stitched_granularity(int device, size_t* bytes);
 int sap_stitched_alloc(int32_t n_chunks, size_t chunk_bytes, const int32_t* device_of_chunk, int32_t n_access,
@@ -284,6 +285,14 @@ void* sap_stitched_ptr(const sap_stitched_t* s);            /* device pointer of
 size_t sap_stitched_bytes(const sap_stitched_t* s);         /* n_chunks * chunk_bytes */
 int32_t sap_stitched_owner(const sap_stitched_t* s, int32_t chunk);   /* device that holds chunk, -1 if out of range */
 void sap_stitched_free(sap_stitched_t* s);
+/* The same range with one process per GPU (the launch model of torch.distributed): every process reserves the whole
+ * range on its `device`, creates and maps the chunks c with own[c] != 0 (host array [n_chunks]) as exportable allocations,
+ * hands a POSIX file descriptor of each to the other processes (sap_stitched_export_fd; the descriptor travels over a Unix
+ * socket with SCM_RIGHTS, the receiver closes it after the import) and maps theirs (sap_stitched_import_fd, chunk not yet
+ * mapped).  A chunk that is not mapped must not be touched.  sap_stitched_owner is -1 for imported chunks.  Synchronous. */
+int sap_stitched_create_local(int32_t n_chunks, size_t chunk_bytes, int device, const uint8_t* own, sap_stitched_t** out);
+int sap_stitched_export_fd(const sap_stitched_t* s, int32_t chunk, int* fd);
+int sap_stitched_import_fd(sap_stitched_t* s, int32_t chunk, int fd);
 
 const char* sap_strerror(int status);
 int sap_last_cuda_error(void);      /* the cudaError_t / CUresult of the last SAP_ERR_CUDA on this thread */

@@ -64,6 +64,10 @@ SIGNATURES = {
     "sap_stitched_bytes": (ctypes.c_size_t, [vp]),
     "sap_stitched_owner": (ctypes.c_int32, [vp, ctypes.c_int32]),
     "sap_stitched_free": (None, [vp]),
+    "sap_stitched_create_local": (ctypes.c_int, [ctypes.c_int32, ctypes.c_size_t, ctypes.c_int, ctypes.POINTER(ctypes.c_uint8),
+                                                 ctypes.POINTER(vp)]),
+    "sap_stitched_export_fd": (ctypes.c_int, [vp, ctypes.c_int32, ctypes.POINTER(ctypes.c_int)]),
+    "sap_stitched_import_fd": (ctypes.c_int, [vp, ctypes.c_int32, ctypes.c_int]),
     "sap_strerror": (ctypes.c_char_p, [ctypes.c_int]),
     "sap_last_cuda_error": (ctypes.c_int, []),
     "sap_launch_count": (ctypes.c_int64, []),

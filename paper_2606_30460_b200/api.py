@@ -352,6 +352,28 @@ class Stitched:
         self.nbytes = int(_lib.lib().sap_stitched_bytes(self.handle))
         self.n_chunks, self.chunk_bytes, self.devices = int(n_chunks), int(chunk_bytes), devices
 
+    @classmethod
+    def create_local(cls, n_chunks: int, chunk_bytes: int, device: int, own: Sequence[bool]) -> "Stitched":
+        """One process per GPU: reserve the whole range on `device`, create (exportable) and map the chunks with own[c];
+        the others are mapped later with import_fd from their owners' export_fd descriptors."""
+        self = cls.__new__(cls)
+        self.handle = ctypes.c_void_p()
+        mask = (ctypes.c_uint8 * int(n_chunks))(*[1 if o else 0 for o in own])
+        _check(_lib.lib().sap_stitched_create_local(int(n_chunks), int(chunk_bytes), int(device), mask,
+                                                    ctypes.byref(self.handle)), "sap_stitched_create_local")
+        self.ptr = int(_lib.lib().sap_stitched_ptr(self.handle))
+        self.nbytes = int(_lib.lib().sap_stitched_bytes(self.handle))
+        self.n_chunks, self.chunk_bytes, self.devices = int(n_chunks), int(chunk_bytes), [int(device)] * int(n_chunks)
+        return self
+
+    def export_fd(self, chunk: int) -> int:
+        fd = ctypes.c_int(-1)
+        _check(_lib.lib().sap_stitched_export_fd(self.handle, int(chunk), ctypes.byref(fd)), "sap_stitched_export_fd")
+        return int(fd.value)
+
+    def import_fd(self, chunk: int, fd: int) -> None:
+        _check(_lib.lib().sap_stitched_import_fd(self.handle, int(chunk), int(fd)), "sap_stitched_import_fd")
+
     @staticmethod
     def granularity(device: int = 0) -> int:
         g = ctypes.c_size_t()

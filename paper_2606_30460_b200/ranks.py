@@ -15,8 +15,9 @@ Control flow = four phases with two group barriers (stream events; no kernel eve
               every rank: sap_attn_bwd_end(own dQ rows)
 Ranks that share a device share its stream (their launches run one after the other): with every chunk on device 0 this
 is the one-GPU emulation the tests run; with distinct P2P-capable devices it is the multi-GPU form - not run anywhere
-yet (no box with a second GPU), so treat that path as untested.  One process drives all devices; the one-process-per-GPU
-form needs the stitched handles exported between processes, which is not built.
+yet (no box with a second GPU), so treat that path as untested.  `RankGroup` drives all devices from one process;
+`ProcessRank` is the one-process-per-GPU form (the stitched ranges are assembled from chunks the processes export to
+one another, the barriers are group barriers): tested with two processes on the one GPU of the box.
 """
 from __future__ import annotations
 
@@ -126,3 +127,162 @@ class RankGroup:
         self._each_rank(lambda c, plan, cu, st: api.sap_attn_bwd_end(plan, c, c + 1, dq, n_kv_heads, workspace,
                                                                      softmax_scale=softmax_scale, stream=st))
         self._join()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# One process per GPU (the launch model of torch.distributed): the same phases, the barriers are group barriers of the
+# process group, and the stitched ranges are assembled from chunks the processes export to one another.
+def exchange_fds(rank: int, world: int, my_fds: Dict[int, int], group=None, tag: str = "sap") -> Dict[int, Dict[int, int]]:
+    """Every rank hands the file descriptors `my_fds` (key -> fd, e.g. the exported chunks it owns) to every other
+    rank: descriptors only travel between processes of one host over a Unix socket (SCM_RIGHTS).  Returns
+    {sender rank: {key: fd valid in THIS process}}; the receiver closes them once imported.  Needs an initialised
+    torch.distributed group (any backend: used for two barriers only)."""
+    import array
+    import os
+    import socket
+    import struct
+    import tempfile
+    import torch.distributed as dist
+
+    if world == 1:
+        return {}
+    base = os.path.join(tempfile.gettempdir(), f"{tag}_fd_{os.environ.get('MASTER_PORT', '0')}_")
+    path = base + str(rank)
+    if os.path.exists(path):
+        os.unlink(path)
+    srv = socket.socket(socket.AF_UNIX, socket.SOCK_STREAM)
+    srv.bind(path)
+    srv.listen(world)
+    dist.barrier(group=group)                      # every rank listens
+    keys = sorted(my_fds)
+    for peer in range(world):                      # send to everybody (small messages: the connects do not block)
+        if peer == rank:
+            continue
+        c = socket.socket(socket.AF_UNIX, socket.SOCK_STREAM)
+        c.connect(base + str(peer))
+        payload = struct.pack(f"<ii{len(keys)}i", rank, len(keys), *keys)
+        fds = array.array("i", [my_fds[k] for k in keys])
+        c.sendmsg([payload], [(socket.SOL_SOCKET, socket.SCM_RIGHTS, fds)] if keys else [])
+        c.close()
+    got: Dict[int, Dict[int, int]] = {}
+    for _ in range(world - 1):
+        conn, _addr = srv.accept()
+        msg, anc, _flags, _a = conn.recvmsg(4096, socket.CMSG_SPACE(4 * 256))
+        sender, n = struct.unpack_from("<ii", msg)
+        ks = struct.unpack_from(f"<{n}i", msg, 8)
+        fds = array.array("i")
+        for level, typ, data in anc:
+            if level == socket.SOL_SOCKET and typ == socket.SCM_RIGHTS:
+                fds.frombytes(data[: len(data) - (len(data) % fds.itemsize)])
+        got[sender] = dict(zip(ks, list(fds)))
+        conn.close()
+    dist.barrier(group=group)                      # every rank has received
+    srv.close()
+    os.unlink(path)
+    return got
+
+
+def launch_chunks(rank: int, world: int, n_chunks: int, balance: str = "zigzag") -> List[int]:
+    """The chunks rank `rank` LAUNCHES (its q-chunks in the forward, its kv-chunks in the backward).  With stitched
+    tensors that is independent of whose memory a chunk is, so the causal imbalance of contiguous ownership (the last
+    rank's rows see every chunk, the first rank's only their own; the paper balances it by moving blocks between
+    ranks) is removed by the assignment alone: "zigzag" gives rank r the chunks r, 2W-1-r, 2W+r, ...
+    (a cheap chunk paired with an expensive one); "contiguous" = the chunks whose memory the rank owns."""
+    per = n_chunks // world
+    if balance == "contiguous":
+        return list(range(rank * per, (rank + 1) * per))
+    out = []
+    for lap in range(per):
+        out.append(lap * world + (rank if lap % 2 == 0 else world - 1 - rank))
+    return out
+
+
+class ProcessRank:
+    """This process = SAP rank `rank` of `world` on its own CUDA device.  The sequence has n_chunks chunks (a multiple of
+    world; default one per rank); the rank OWNS the memory of a contiguous block of them and LAUNCHES the
+    chunks `launch_chunks` gives it."""
+
+    def __init__(self, cu_seqlens: Sequence[int], rank: int, world: int, device: int, group=None,
+                 n_chunks: Optional[int] = None, balance: str = "zigzag"):
+        import torch
+        self.rank, self.world, self.device, self.group = int(rank), int(world), int(device), group
+        self.P = int(world if n_chunks is None else n_chunks)
+        if self.P % self.world != 0:
+            raise ValueError("n_chunks must be a multiple of the number of ranks")
+        self.cu_seqlens = list(cu_seqlens)
+        self.n_tokens = int(self.cu_seqlens[-1])
+        torch.cuda.set_device(self.device)
+        self.plan = api.sap_plan(self.cu_seqlens, self.P)
+        self.plan.upload()
+        self.cu_dev = self.plan.cu_seqlens_dev(torch.device("cuda", self.device))
+        per = self.P // self.world
+        self.owned = list(range(self.rank * per, (self.rank + 1) * per))
+        self.launch = launch_chunks(self.rank, self.world, self.P, balance)
+        self._n_ranges = 0
+
+    def _assemble(self, n_chunks: int, chunk_bytes: int, own: Sequence[bool]) -> api.Stitched:
+        import os
+        s = api.Stitched.create_local(n_chunks, chunk_bytes, self.device, own)
+        mine = {c: s.export_fd(c) for c in range(n_chunks) if own[c]}
+        self._n_ranges += 1
+        theirs = exchange_fds(self.rank, self.world, mine, self.group, tag=f"sap{self._n_ranges}")
+        for _sender, fds in theirs.items():
+            for c, fd in fds.items():
+                s.import_fd(c, fd)
+                os.close(fd)
+        for fd in mine.values():
+            os.close(fd)
+        return s
+
+    def tensor(self, tail_shape: Sequence[int], dtype):
+        """[N, *tail_shape]: rows of chunk c are memory of the process that owns chunk c, mapped into this one."""
+        import torch
+        row = 1
+        for x in tail_shape:
+            row *= int(x)
+        chunk_bytes = (self.n_tokens // self.P) * row * torch.empty((), dtype=dtype).element_size()
+        s = self._assemble(self.P, chunk_bytes, [c in self.owned for c in range(self.P)])
+        return s.tensor((self.n_tokens, *tail_shape), dtype, device=f"cuda:{self.device}")
+
+    def own_rows(self) -> slice:
+        n = self.n_tokens // self.P
+        return slice(self.owned[0] * n, (self.owned[-1] + 1) * n)
+
+    def shared(self, shape: Sequence[int], dtype):
+        """One array for all ranks ([Hq, N] LSE, the backward workspace): memory of rank 0, mapped by every rank."""
+        import torch
+        nbytes = torch.empty((), dtype=dtype).element_size()
+        for x in shape:
+            nbytes *= int(x)
+        g = api.Stitched.granularity(self.device)
+        s = self._assemble(1, (nbytes + g - 1) // g * g, [self.rank == 0])
+        return s.tensor(tuple(shape), dtype, device=f"cuda:{self.device}")
+
+    def workspace(self, n_q_heads: int, n_kv_heads: int, head_dim: int):
+        import torch
+        return self.shared((api.sap_workspace_bytes(self.plan, n_q_heads, n_kv_heads, head_dim, api.SAP_PASS_BWD),), torch.uint8)
+
+    def barrier(self):
+        """Group barrier between phases: this rank's launches have finished and so have everybody else's."""
+        import torch
+        import torch.distributed as dist
+        torch.cuda.synchronize()
+        if self.world > 1:
+            dist.barrier(group=self.group)
+
+    def forward(self, q, k, v, out, lse, softmax_scale: Optional[float] = None):
+        for c in self.launch:
+            api.sap_attn_fwd_chunks(q, k, v, self.cu_dev, self.plan, c, c + 1, out, lse, softmax_scale=softmax_scale)
+
+    def backward(self, dout, q, k, v, out, lse, dq, dk, dv, workspace, softmax_scale: Optional[float] = None):
+        n_kv_heads = k.shape[1]
+        self.barrier()         # every forward row (out, LSE) is written
+        for c in self.launch:
+            api.sap_attn_bwd_begin(dout, out, self.plan, c, c + 1, n_kv_heads, workspace)
+        self.barrier()         # every D written, every accumulator row zeroed
+        for c in self.launch:
+            api.sap_attn_bwd_chunks(dout, q, k, v, lse, self.cu_dev, self.plan, c, c + 1, dk, dv, workspace, softmax_scale=softmax_scale)
+        self.barrier()         # every dQ contribution added
+        for c in self.launch:
+            api.sap_attn_bwd_end(self.plan, c, c + 1, dq, n_kv_heads, workspace, softmax_scale=softmax_scale)
+        self.barrier()

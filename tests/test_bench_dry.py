@@ -20,7 +20,7 @@ def run_bench(*extra):
     return json.loads(lines[0])
 
 
-@pytest.mark.parametrize("shard, scaling", [("seqs", "weak"), ("heads", "strong")])
+@pytest.mark.parametrize("shard, scaling", [("seqs", "weak"), ("heads", "strong"), ("chunks", "strong")])
 def test_bench_gpus_2_spawns_two_ranks(shard, scaling):
     one = run_bench("--shard", shard)
     two = run_bench("--gpus", "2", "--shard", shard)
@@ -28,6 +28,9 @@ def test_bench_gpus_2_spawns_two_ranks(shard, scaling):
     assert two["max_over_ranks_check"] is True               # the MAX-over-ranks all-reduce saw both ranks
     if shard == "heads":                                     # one sequence split by kv-heads: the same total work
         assert two["kv_heads_of_rank0"] == [0, 1, 2, 3]
+        assert two["whole_job_tflop_per_step"] == pytest.approx(one["whole_job_tflop_per_step"])
+    elif shard == "chunks":                                  # one sequence split by chunks (the paper's SP): zig-zag launches
+        assert two["chunks_launched_by_rank"] == [[0, 3, 4, 7], [1, 2, 5, 6]]
         assert two["whole_job_tflop_per_step"] == pytest.approx(one["whole_job_tflop_per_step"])
     else:                                                    # independent sequences: work adds up (different seeds)
         assert two["whole_job_tflop_per_step"] > one["whole_job_tflop_per_step"]
