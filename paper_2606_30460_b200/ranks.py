@@ -26,6 +26,19 @@ from typing import Dict, List, Optional, Sequence
 from . import api
 
 
+def workspace_units(n_tokens: int, n_chunks: int, n_q_heads: int, head_dim: int, granularity: int):
+    """Layout of the backward workspace (sap_workspace_bytes: D fp32 [Hq, N] padded to 256 B, then the fp32 dQ accumulator
+    [N, Hq, d]) as equal units of a stitched range, so that the accumulator rows of chunk c can live with the owner of
+    chunk c - the dQ contributions of every rank (red.global) then land in the memory of the rank that will read them,
+    not in one rank's.  Returns (unit_bytes, units_per_chunk) with unit 0 = the D array, or None when the sizes do not
+    line up (D not a multiple of the allocation granularity, or a chunk's accumulator not a multiple of D)."""
+    d_bytes = (n_tokens * n_q_heads * 4 + 255) // 256 * 256
+    acc_chunk = (n_tokens // n_chunks) * n_q_heads * head_dim * 4
+    if d_bytes % granularity != 0 or acc_chunk % d_bytes != 0:
+        return None
+    return d_bytes, acc_chunk // d_bytes
+
+
 class RankGroup:
     def __init__(self, cu_seqlens: Sequence[int], n_chunks: int, devices: Optional[Sequence[int]] = None):
         import torch
@@ -71,9 +84,17 @@ class RankGroup:
         return s.tensor(tuple(shape), dtype)
 
     def workspace(self, n_q_heads: int, n_kv_heads: int, head_dim: int):
+        """The backward workspace; the accumulator rows of chunk c on devices[c] when the sizes line up (workspace_units)."""
         import torch
         plan = self.plans[self.devices[0]]
-        return self.shared((api.sap_workspace_bytes(plan, n_q_heads, n_kv_heads, head_dim, api.SAP_PASS_BWD),), torch.uint8)
+        nbytes = api.sap_workspace_bytes(plan, n_q_heads, n_kv_heads, head_dim, api.SAP_PASS_BWD)
+        lay = workspace_units(self.n_tokens, self.P, n_q_heads, head_dim, api.Stitched.granularity(self.devices[0]))
+        if lay is None:
+            return self.shared((nbytes,), torch.uint8)
+        unit, per = lay
+        owners = [self.devices[0]] + [self.devices[c] for c in range(self.P) for _ in range(per)]
+        s = api.Stitched(len(owners), unit, owners, sorted(set(self.devices)))
+        return s.tensor((nbytes,), torch.uint8)
 
     # ------------------------------------------------------------------ control
     def _fork(self):
@@ -259,8 +280,17 @@ class ProcessRank:
         return s.tensor(tuple(shape), dtype, device=f"cuda:{self.device}")
 
     def workspace(self, n_q_heads: int, n_kv_heads: int, head_dim: int):
+        """The backward workspace; the accumulator rows of chunk c in the memory of the process that owns chunk c when the
+        sizes line up (workspace_units), else one array in rank 0's memory."""
         import torch
-        return self.shared((api.sap_workspace_bytes(self.plan, n_q_heads, n_kv_heads, head_dim, api.SAP_PASS_BWD),), torch.uint8)
+        nbytes = api.sap_workspace_bytes(self.plan, n_q_heads, n_kv_heads, head_dim, api.SAP_PASS_BWD)
+        lay = workspace_units(self.n_tokens, self.P, n_q_heads, head_dim, api.Stitched.granularity(self.device))
+        if lay is None:
+            return self.shared((nbytes,), torch.uint8)
+        unit, per = lay
+        own = [self.rank == 0] + [c in self.owned for c in range(self.P) for _ in range(per)]
+        s = self._assemble(len(own), unit, own)
+        return s.tensor((nbytes,), torch.uint8, device=f"cuda:{self.device}")
 
     def barrier(self):
         """Group barrier between phases: this rank's launches have finished and so have everybody else's."""

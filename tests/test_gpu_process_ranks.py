@@ -31,7 +31,8 @@ def _worker(rank, world, port, result_q):
         from paper_2606_30460_b200.ranks import ProcessRank
         from paper_2606_30460_b200.workloads import custom_workload, make_qkv
         from parity import check_close, to_np
-        w = custom_workload([9000, 5000, 2384], 4, 4, 2, 128, name="process_ranks")      # 16384 tokens, 4 chunks of 4096
+        # 65536 tokens, 4 chunks of 16384, 8 / 2 heads: D is 2 MiB, so the dQ accumulator can live with the chunk owners
+        w = custom_workload([30000, 20000, 15536], 4, 8, 2, 128, name="process_ranks")
         Hq, Hkv, d = w.n_q_heads, w.n_kv_heads, w.head_dim
         q, k, v, do = make_qkv(w, device="cuda")                  # every process can generate the (seeded) inputs
         # two chunks of memory per rank (rank 0: chunks 0-1, rank 1: chunks 2-3); launches zig-zag: rank 0 chunks 0 and 3,
@@ -41,7 +42,9 @@ def _worker(rank, world, port, result_q):
         sq, sdo, so, sdq = (pr.tensor((Hq, d), torch.bfloat16) for _ in range(4))
         sk, sv, sdk, sdv = (pr.tensor((Hkv, d), torch.bfloat16) for _ in range(4))
         slse = pr.shared((Hq, w.n_tokens), torch.float32)
-        ws = pr.workspace(Hq, Hkv, d)
+        from paper_2606_30460_b200.ranks import workspace_units
+        assert workspace_units(w.n_tokens, w.n_chunks, Hq, d, sap.Stitched.granularity(0)) == (2 << 20, 32)
+        ws = pr.workspace(Hq, Hkv, d)                             # accumulator rows of chunk c in the memory of c's owner
         rows = pr.own_rows()
         for dst, src in ((sq, q), (sk, k), (sv, v), (sdo, do)):    # a rank fills only the rows it owns
             dst[rows].copy_(src[rows])
