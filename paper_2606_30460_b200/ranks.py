@@ -300,19 +300,30 @@ class ProcessRank:
         if self.world > 1:
             dist.barrier(group=self.group)
 
+    def _ranges(self):
+        """The launched chunks as [begin, end) runs: neighbours (7 and 8 of a zig-zag lap) share one launch."""
+        runs, cs = [], sorted(self.launch)
+        for c in cs:
+            if runs and runs[-1][1] == c:
+                runs[-1][1] = c + 1
+            else:
+                runs.append([c, c + 1])
+        return [(a, b) for a, b in runs]
+
     def forward(self, q, k, v, out, lse, softmax_scale: Optional[float] = None):
-        for c in self.launch:
-            api.sap_attn_fwd_chunks(q, k, v, self.cu_dev, self.plan, c, c + 1, out, lse, softmax_scale=softmax_scale)
+        for a, b in self._ranges():
+            api.sap_attn_fwd_chunks(q, k, v, self.cu_dev, self.plan, a, b, out, lse, softmax_scale=softmax_scale)
 
     def backward(self, dout, q, k, v, out, lse, dq, dk, dv, workspace, softmax_scale: Optional[float] = None):
         n_kv_heads = k.shape[1]
         self.barrier()         # every forward row (out, LSE) is written
-        for c in self.launch:
-            api.sap_attn_bwd_begin(dout, out, self.plan, c, c + 1, n_kv_heads, workspace)
+        runs = self._ranges()
+        for a, b in runs:
+            api.sap_attn_bwd_begin(dout, out, self.plan, a, b, n_kv_heads, workspace)
         self.barrier()         # every D written, every accumulator row zeroed
-        for c in self.launch:
-            api.sap_attn_bwd_chunks(dout, q, k, v, lse, self.cu_dev, self.plan, c, c + 1, dk, dv, workspace, softmax_scale=softmax_scale)
+        for a, b in runs:
+            api.sap_attn_bwd_chunks(dout, q, k, v, lse, self.cu_dev, self.plan, a, b, dk, dv, workspace, softmax_scale=softmax_scale)
         self.barrier()         # every dQ contribution added
-        for c in self.launch:
-            api.sap_attn_bwd_end(self.plan, c, c + 1, dq, n_kv_heads, workspace, softmax_scale=softmax_scale)
+        for a, b in runs:
+            api.sap_attn_bwd_end(self.plan, a, b, dq, n_kv_heads, workspace, softmax_scale=softmax_scale)
         self.barrier()
