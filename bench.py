@@ -260,10 +260,14 @@ def run_dry(args):
         dist.init_process_group("gloo")
     extra = {}
     if args.shard == "chunks":       # one sequence, every head, rank r launches the chunks ranks.launch_chunks gives it
-        from paper_2606_30460_b200.ranks import launch_chunks
+        from paper_2606_30460_b200.ranks import assign_by_work, chunk_work
         w = shard.rank_workload(args.config, 0)
         heads, share = tuple(range(w.n_kv_heads)), 1.0 / world
-        extra = {"chunks_launched_by_rank": [launch_chunks(r, world, w.n_chunks) for r in range(world)]}
+        q_work, kv_work = chunk_work(w.cu_seqlens, w.n_chunks)
+        fwd_a, bwd_a = assign_by_work(q_work, world), assign_by_work(kv_work, world)
+        extra = {"q_chunks_launched_by_rank": fwd_a, "kv_chunks_launched_by_rank": bwd_a,
+                 "max_over_mean_load": {"fwd": max(sum(q_work[c] for c in x) for x in fwd_a) * world / sum(q_work),
+                                        "bwd": max(sum(kv_work[c] for c in x) for x in bwd_a) * world / sum(kv_work)}}
     else:
         w, heads = shard.rank_share(args.config, rank, world, args.shard)
         share = len(heads) / w.n_kv_heads
@@ -283,7 +287,7 @@ def run_dry(args):
 def run_chunks(args):
     """`--shard chunks`: the paper's sequence parallelism itself.  ONE packed sequence; rank r owns the
     memory of a contiguous block of its chunks (stitched tensors: ranks.ProcessRank) and launches the library's kernels on
-    the chunks the zig-zag assignment gives it; K/V, Q/dO and the dQ contributions travel inside the kernels (TMA and
+    the chunks a work-balanced assignment gives it (visible pairs per chunk, from cu_seqlens); K/V, Q/dO and the dQ contributions travel inside the kernels (TMA and
     red.global over NVLink), the only synchronisation is four group barriers per step.  Strong scaling.  A step also
     includes, under `e2e`, every rank's own rows going host -> device and its results coming back."""
     import torch
@@ -363,8 +367,9 @@ def run_chunks(args):
             "data": "synthetic",
             "config": {"workload": w.name, "n_tokens": N, "n_docs": len(w.doc_lens), "n_chunks": w.n_chunks, "n_q_heads": Hq,
                        "n_kv_heads": Hkv, "head_dim": d, "cu_seqlens_sha256": w.sha256(), "shard": "chunks",
-                       "per_rank": "one sequence; rank r owns the memory of chunks %s.. and launches %s (zig-zag); stitched tensors, "
-                                   "4 group barriers per step, no collective on the data path" % (pr.owned[0], pr.launch),
+                       "per_rank": "one sequence; rank 0 owns the memory of chunks %s and launches q-chunks %s / kv-chunks %s (balanced by "
+                                   "visible pairs); stitched tensors, 4 group barriers per step, no collective on the data path"
+                                   % (pr.owned, pr.launch, pr.launch_kv),
                        "l2": "inputs exceed L2"},
             "frac_of_bf16_peak": {"measured_burst": value / world / peaks["bf16_burst"],
                                   "measured_sustained": value / world / peaks["bf16_sustained"], "source": peaks["source"]},

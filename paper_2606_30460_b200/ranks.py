@@ -218,13 +218,42 @@ def launch_chunks(rank: int, world: int, n_chunks: int, balance: str = "zigzag")
     return out
 
 
+def chunk_work(cu_seqlens: Sequence[int], n_chunks: int):
+    """Visible (row, key) pairs per q-chunk (the rows of the chunk: what a forward launch on it computes) and per kv-chunk
+    (the keys of the chunk: what a backward launch on it computes), from cu_seqlens alone: row t sees t - start(doc(t)) + 1
+    keys, key s is seen by end(doc(s)) - s rows."""
+    import numpy as np
+    cu = np.asarray(cu_seqlens, dtype=np.int64)
+    N = int(cu[-1])
+    t = np.arange(N, dtype=np.int64)
+    doc = np.searchsorted(cu, t, side="right") - 1
+    n = N // n_chunks
+    q_work = (t - cu[doc] + 1).reshape(n_chunks, n).sum(axis=1)
+    kv_work = (cu[doc + 1] - t).reshape(n_chunks, n).sum(axis=1)
+    return [int(x) for x in q_work], [int(x) for x in kv_work]
+
+
+def assign_by_work(work: Sequence[int], world: int) -> List[List[int]]:
+    """Longest-processing-time greedy: chunks in order of decreasing work (lower index first on ties), each to the rank
+    with the least work so far (lowest rank on ties).  Deterministic: every rank computes the same assignment."""
+    load = [0] * world
+    out: List[List[int]] = [[] for _ in range(world)]
+    for c in sorted(range(len(work)), key=lambda c: (-work[c], c)):
+        r = min(range(world), key=lambda r: (load[r], r))
+        out[r].append(c)
+        load[r] += work[c]
+    return [sorted(x) for x in out]
+
+
 class ProcessRank:
     """This process = SAP rank `rank` of `world` on its own CUDA device.  The sequence has n_chunks chunks (a multiple of
     world; default one per rank); the rank OWNS the memory of a contiguous block of them and LAUNCHES the
-    chunks `launch_chunks` gives it."""
+    chunks the balance policy gives it: "work" (default) = by the visible pairs of each chunk, computed from cu_seqlens
+    (the compile-time information of PAPER.md:106), separately for the forward (q-chunks) and the backward (kv-chunks);
+    "zigzag" / "contiguous" = `launch_chunks`."""
 
     def __init__(self, cu_seqlens: Sequence[int], rank: int, world: int, device: int, group=None,
-                 n_chunks: Optional[int] = None, balance: str = "zigzag"):
+                 n_chunks: Optional[int] = None, balance: str = "work"):
         import torch
         self.rank, self.world, self.device, self.group = int(rank), int(world), int(device), group
         self.P = int(world if n_chunks is None else n_chunks)
@@ -238,7 +267,13 @@ class ProcessRank:
         self.cu_dev = self.plan.cu_seqlens_dev(torch.device("cuda", self.device))
         per = self.P // self.world
         self.owned = list(range(self.rank * per, (self.rank + 1) * per))
-        self.launch = launch_chunks(self.rank, self.world, self.P, balance)
+        if balance == "work":
+            q_work, kv_work = chunk_work(self.cu_seqlens, self.P)
+            self.launch = assign_by_work(q_work, self.world)[self.rank]        # forward, D pre-pass, dQ post pass: q-chunks
+            self.launch_kv = assign_by_work(kv_work, self.world)[self.rank]    # backward main kernel: kv-chunks
+        else:
+            self.launch = launch_chunks(self.rank, self.world, self.P, balance)
+            self.launch_kv = list(self.launch)
         self._n_ranges = 0
 
     def _assemble(self, n_chunks: int, chunk_bytes: int, own: Sequence[bool]) -> api.Stitched:
@@ -300,9 +335,10 @@ class ProcessRank:
         if self.world > 1:
             dist.barrier(group=self.group)
 
-    def _ranges(self):
-        """The launched chunks as [begin, end) runs: neighbours (7 and 8 of a zig-zag lap) share one launch."""
-        runs, cs = [], sorted(self.launch)
+    @staticmethod
+    def _ranges(chunks):
+        """Chunks as [begin, end) runs: neighbours (7 and 8 of a zig-zag lap) share one launch."""
+        runs, cs = [], sorted(chunks)
         for c in cs:
             if runs and runs[-1][1] == c:
                 runs[-1][1] = c + 1
@@ -311,17 +347,17 @@ class ProcessRank:
         return [(a, b) for a, b in runs]
 
     def forward(self, q, k, v, out, lse, softmax_scale: Optional[float] = None):
-        for a, b in self._ranges():
+        for a, b in self._ranges(self.launch):
             api.sap_attn_fwd_chunks(q, k, v, self.cu_dev, self.plan, a, b, out, lse, softmax_scale=softmax_scale)
 
     def backward(self, dout, q, k, v, out, lse, dq, dk, dv, workspace, softmax_scale: Optional[float] = None):
         n_kv_heads = k.shape[1]
         self.barrier()         # every forward row (out, LSE) is written
-        runs = self._ranges()
+        runs = self._ranges(self.launch)
         for a, b in runs:
             api.sap_attn_bwd_begin(dout, out, self.plan, a, b, n_kv_heads, workspace)
         self.barrier()         # every D written, every accumulator row zeroed
-        for a, b in runs:
+        for a, b in self._ranges(self.launch_kv):
             api.sap_attn_bwd_chunks(dout, q, k, v, lse, self.cu_dev, self.plan, a, b, dk, dv, workspace, softmax_scale=softmax_scale)
         self.barrier()         # every dQ contribution added
         for a, b in runs:

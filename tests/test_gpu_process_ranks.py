@@ -35,10 +35,11 @@ def _worker(rank, world, port, result_q):
         w = custom_workload([30000, 20000, 15536], 4, 8, 2, 128, name="process_ranks")
         Hq, Hkv, d = w.n_q_heads, w.n_kv_heads, w.head_dim
         q, k, v, do = make_qkv(w, device="cuda")                  # every process can generate the (seeded) inputs
-        # two chunks of memory per rank (rank 0: chunks 0-1, rank 1: chunks 2-3); launches zig-zag: rank 0 chunks 0 and 3,
-        # rank 1 chunks 1 and 2 - every rank launches on a chunk whose memory belongs to the other process
+        # two chunks of memory per rank (rank 0: chunks 0-1, rank 1: chunks 2-3); the launches are balanced by visible pairs
+        # (separately for q-chunks and kv-chunks), so a rank also launches on chunks whose memory belongs to the other process
         pr = ProcessRank(w.cu_seqlens, rank, world, device=0, n_chunks=w.n_chunks)
-        assert pr.launch == ([0, 3] if rank == 0 else [1, 2]) and pr.owned == ([0, 1] if rank == 0 else [2, 3])
+        assert pr.owned == ([0, 1] if rank == 0 else [2, 3])
+        assert set(pr.launch) != set(pr.owned) or set(pr.launch_kv) != set(pr.owned)
         sq, sdo, so, sdq = (pr.tensor((Hq, d), torch.bfloat16) for _ in range(4))
         sk, sv, sdk, sdv = (pr.tensor((Hkv, d), torch.bfloat16) for _ in range(4))
         slse = pr.shared((Hq, w.n_tokens), torch.float32)

@@ -65,3 +65,24 @@ def test_launch_chunks_cover_every_chunk_once_and_balance_the_causal_load():
         if (P // world) % 2 == 0:
             assert max(zz) == min(zz) and max(ct) > min(ct)
         assert max(zz) <= max(ct)
+
+
+def test_work_balanced_assignment():
+    """ranks.chunk_work / assign_by_work: the per-chunk work sums to the useful pairs of the sequence (both ways of
+    counting), the assignment is a partition, and greedy LPT is within one chunk's work of the mean."""
+    from paper_2606_30460_b200.ranks import assign_by_work, chunk_work
+    from paper_2606_30460_b200.workloads import make_workload
+    for cfg in (1, 2, 3, 4, 5):
+        w = make_workload(cfg)
+        q_work, kv_work = chunk_work(w.cu_seqlens, w.n_chunks)
+        assert sum(q_work) == w.pairs == sum(kv_work)
+        for world in (1, 2, 4):
+            for work in (q_work, kv_work):
+                a = assign_by_work(work, world)
+                assert sorted(sum(a, [])) == list(range(w.n_chunks))
+                loads = [sum(work[c] for c in x) for x in a]
+                assert max(loads) - min(loads) <= max(work)
+    # one document: q-chunk c costs about (2c + 1) blocks; LPT pairs cheap with expensive chunks like zig-zag does
+    q_work, _ = chunk_work([0, 8192], 8)
+    loads = [sum(q_work[c] for c in x) for x in assign_by_work(q_work, 4)]
+    assert max(loads) / (sum(loads) / 4) < 1.01
