@@ -450,8 +450,21 @@ def run_ours(args):
     if rank == 0:
         sampler.start()
     launches0 = sap.sap_launch_count()
-    ms = timed(step, args.steps)
-    launches = sap.sap_launch_count() - launches0
+    if args.graph:   # launch-bound shapes: the whole step captured once (no call allocates or synchronises), replayed K times
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(side):
+            with torch.cuda.graph(graph, stream=side):
+                step()
+        per_step = sap.sap_launch_count() - launches0
+        torch.cuda.current_stream().wait_stream(side)
+        graph.replay(); torch.cuda.synchronize()
+        ms = timed(graph.replay, args.steps)
+        launches = per_step * args.steps
+    else:
+        ms = timed(step, args.steps)
+        launches = sap.sap_launch_count() - launches0
     sync_all()
     clocks = sampler.stop() if rank == 0 else None
     ms_max, flops_all = shard.aggregate(ms, float(w.flops_fwd + w.flops_bwd) * share, dev)   # MAX time, SUM work
@@ -485,7 +498,7 @@ def run_ours(args):
             bwd_ms = sum(per.values())
             print(json.dumps({"profile_only": True, "workload": w.name, "n_tokens": N, "n_docs": len(w.doc_lens),
                               "useful_pairs": w.pairs, "plan_items": plan.n_items, "cu_seqlens_sha256": w.sha256(), "shard": args.shard, "n_gpus": world,
-                              "bwd": args.bwd, "ms_per_step": ms_max, "value": value,
+                              "bwd": args.bwd, "cuda_graph": bool(args.graph), "ms_per_step": ms_max, "value": value,
                               "frac_of_measured_burst_peak": value / world / load_peaks()["bf16_burst"],
                               "tokens_per_s": N * world / (ms_max * 1e-3), "fwd_ms": t_fwd,
                               "fwd_tflops": w.flops_fwd * share / (t_fwd * 1e-3) / 1e12, "bwd_ms": bwd_ms,
@@ -607,7 +620,7 @@ def run_ours(args):
                        "plan_items": plan.n_items, "l2": "inputs exceed L2 (Q alone is %.0f MiB)" % (q.numel() * 2 / 2**20),
                        "per_rank": ("independent sequence per rank (seed = rank)" if args.shard == "seqs" else
                                     f"one sequence, {Hkv} of its {w.n_kv_heads} kv-heads (and their q-heads) per rank, no exchange"),
-                       "shard": args.shard, "bwd": args.bwd},
+                       "shard": args.shard, "bwd": args.bwd, "cuda_graph": bool(args.graph)},
             "tokens_per_s": N * world / (ms_max * 1e-3),
             "frac_of_bf16_peak": {"measured_burst": value / world / peaks["bf16_burst"],
                                   "measured_sustained": value / world / peaks["bf16_sustained"],
@@ -648,6 +661,7 @@ def main():
     ap.add_argument("--shard", default="seqs", choices=["seqs", "heads", "chunks"],
                     help="multi-GPU split: independent sequences per rank (weak scaling), the kv-heads of one sequence (strong), or "
                          "the chunks of one sequence = the paper's sequence parallelism over stitched tensors (strong)")
+    ap.add_argument("--graph", action="store_true", help="time replays of one captured CUDA graph of the step (launch-bound shapes)")
     ap.add_argument("--dry-run", action="store_true", help="host side only (planner, sharding, aggregation over gloo); no GPU")
     ap.add_argument("--profile-only", action="store_true",
                     help="stop after the device-timed region and the per-kernel passes (for ncu runs)")

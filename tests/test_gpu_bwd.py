@@ -102,3 +102,38 @@ def test_bwd_workspace_too_small():
     with pytest.raises(sap.SapError) as e:
         sap.sap_attn_bwd(do, q, k, v, out, lse, cu, plan, workspace=torch.empty(16, dtype=torch.uint8, device="cuda"))
     assert e.value.status == 5
+
+
+def test_step_is_capturable_into_a_cuda_graph():
+    """No attention call allocates, synchronises or reads device state on the host (sap.h: asynchronous on the caller's
+    stream), so a whole step - forward, D pre-pass, accumulator zeroing, backward main kernel, dQ post pass - can be
+    captured once and replayed: the replay must reproduce the eager results (forward, dK, dV bit for bit; dQ within
+    tolerance: its accumulation is atomic).  The small, launch-bound shapes are where that pays."""
+    w = custom_workload([700, 1100, 248], 4, 8, 2, 128, name="graph")
+    q, k, v, do = make_qkv(w, device="cuda")
+    plan = sap.sap_plan(w.cu_seqlens, w.n_chunks)
+    plan.upload()
+    cu = plan.cu_seqlens_dev("cuda")
+    ws = torch.empty(sap.sap_workspace_bytes(plan, w.n_q_heads, w.n_kv_heads, w.head_dim, sap.SAP_PASS_BWD), dtype=torch.uint8,
+                     device="cuda")
+    out, lse = sap.sap_attn_fwd(q, k, v, cu, plan, softmax_scale=w.softmax_scale)
+    dq, dk, dv = sap.sap_attn_bwd(do, q, k, v, out, lse, cu, plan, softmax_scale=w.softmax_scale, workspace=ws)
+    torch.cuda.synchronize()
+    g_out, g_lse = torch.empty_like(out), torch.empty_like(lse)
+    g_dq, g_dk, g_dv = torch.empty_like(dq), torch.empty_like(dk), torch.empty_like(dv)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            sap.sap_attn_fwd(q, k, v, cu, plan, out=g_out, lse=g_lse, softmax_scale=w.softmax_scale)
+            sap.sap_attn_bwd(do, q, k, v, g_out, g_lse, cu, plan, softmax_scale=w.softmax_scale, dq=g_dq, dk=g_dk, dv=g_dv,
+                             workspace=ws)
+    for rep in range(3):
+        for t in (g_out, g_lse, g_dq, g_dk, g_dv):
+            t.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(g_out, out) and torch.equal(g_lse, lse), f"replay {rep}: forward differs"
+        assert torch.equal(g_dk, dk) and torch.equal(g_dv, dv), f"replay {rep}: dK / dV differ"
+        check_close(to_np(g_dq), to_np(dq), f"replay {rep}: dq")
