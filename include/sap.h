@@ -305,13 +305,16 @@ int64_t sap_launch_count(void);
  * one document and s <= t.  kind: 0 forward (Q-stationary), 1 / 2 backward K/V-stationary with 128- / 256-key tiles;
  * 3 / 4 items [a, b) Q-stationary (all tiles / touched tiles: sap_attn_fwd_partial / sap_attn_fwd_items); 5 q-chunks
  * [a, b) (sap_attn_fwd_chunks); 6 / 7 kv-chunks [a, b) with 128- / 256-key tiles (sap_attn_bwd_chunks); 8 / 9 items
- * [a, b) K/V-stationary (sap_attn_bwd_items).  Returns the number of tiles (call with null buffers to size), *n_segs
+ * [a, b) K/V-stationary (sap_attn_bwd_items); 10 forward with 256-row Q tiles (two 128-row units of one head per work
+ * item: the forward of odd Hq/Hkv, e.g. MHA).  Returns the number of tiles (call with null buffers to size), *n_segs
  * the number of segments; < 0 on error.  Buffers are filled only when large enough. */
 int32_t sap_debug_tile_program(const sap_plan_t* plan, int32_t kind, int32_t a, int32_t b, int32_t* tiles, int32_t tiles_cap,
                                int32_t* segs, int32_t segs_cap, int32_t* n_segs);
-/* Diagnostic: which forward kernel sap_attn_fwd / sap_attn_fwd_partial launch.  0 (default): the pair kernel (two
- * q-heads of one GQA group per CTA, sharing the K/V tiles) whenever Hq/Hkv is even, the one-head kernel otherwise;
- * 1: always the one-head kernel.  Process-wide; returns the previous value. */
+/* Diagnostic: which forward kernel the forward calls launch.  0 (default): the persistent pair kernel on head pairs (two
+ * q-heads of one GQA group per work item, sharing the K/V tiles) whenever Hq/Hkv is even; for odd Hq/Hkv (MHA) the same
+ * kernel on row pairs (two 128-row halves of a 256-row tile of one q-head) in sap_attn_fwd when the launch has at least
+ * 16 work items per SM, the one-head kernel otherwise; 1: always the one-head kernel; 2: row pairs in sap_attn_fwd whatever
+ * the size and Hq/Hkv.  Process-wide; returns the previous value. */
 int sap_debug_set_fwd_form(int form);
 /* Diagnostic: which fused backward main kernel runs at head_dim 128.  0 (default): the CTA-pair kernel (tcgen05
  * cta_group::2 over 256-key pair-tiles); 1: the one-CTA kernel (always used at head_dim 64).  Process-wide; returns the

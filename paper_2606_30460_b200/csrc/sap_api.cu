@@ -163,10 +163,19 @@ static int check_call(sap_plan_t* plan, int64_t n_tokens, int Hq, int Hkv, int d
   return SAP_OK;
 }
 
+// Row pairs pay once there are many work items per SM (measured on the Table 2 shape, 16 heads MHA: 128K tokens 12.27 -> 11.50
+// ms; 32K 0.69 -> 0.70 ms; 8K 0.110 -> 0.117 ms - there the one-head kernel's two smaller CTAs per SM spread the work better).
+static bool use_row_pairs(int n_tiles2, int Hq) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || n_tiles2 <= 0) return false;
+  return static_cast<int64_t>(n_tiles2) * Hq >= 16ll * g_sched[dev].n_sms;
+}
+
+// `prog2` (optional): the same work as `prog` in 256-row Q tiles, for the row-pair form of the pair kernel.
 template <int D, bool PARTIAL>
 static int launch_fwd(const DevProgram& prog, const void* q, const void* k, const void* v, const int32_t* cu,
                       const sap_plan_t* plan, void* out, float* out_f32, float* lse, int Hq, int Hkv, float scale,
-                      cudaStream_t stream) {
+                      cudaStream_t stream, const DevProgram* prog2 = nullptr) {
   if (prog.n_tiles == 0) return SAP_OK;
   CUtensorMap mq, mk, mv;
   int rc;
@@ -181,7 +190,16 @@ static int launch_fwd(const DevProgram& prog, const void* q, const void* k, cons
     const unsigned grid = static_cast<unsigned>(n_work < g_sched[dev].n_sms ? n_work : g_sched[dev].n_sms);
     sap_fwd_pair_kernel<D, PARTIAL><<<grid, kFwdPairThreads, FwdPairSmem<D>::kTotal, stream>>>(
         mq, mk, mv, prog.tiles, prog.segs, cu, plan->n_docs, static_cast<__nv_bfloat16*>(out), out_f32, lse,
-        plan->n_tokens, Hq, Hkv, scale * kLog2e, prog.n_tiles, n_work, next_sched_pair(dev));
+        plan->n_tokens, Hq, Hkv, scale * kLog2e, prog.n_tiles, n_work, next_sched_pair(dev), 0);
+  } else if (prog2 && prog2->n_tiles > 0 && ((g_fwd_form.load() == 0 && use_row_pairs(prog2->n_tiles, Hq)) || g_fwd_form.load() == 2)) {
+    // odd Hq/Hkv (MHA): the same persistent kernel, its two units = the two 128-row halves of a 256-row tile of ONE q-head
+    int dev = 0;
+    SAP_CUDA_CHECK(cudaGetDevice(&dev));
+    const int n_work = prog2->n_tiles * Hq;
+    const unsigned grid = static_cast<unsigned>(n_work < g_sched[dev].n_sms ? n_work : g_sched[dev].n_sms);
+    sap_fwd_pair_kernel<D, PARTIAL><<<grid, kFwdPairThreads, FwdPairSmem<D>::kTotal, stream>>>(
+        mq, mk, mv, prog2->tiles, prog2->segs, cu, plan->n_docs, static_cast<__nv_bfloat16*>(out), out_f32, lse,
+        plan->n_tokens, Hq, Hkv, scale * kLog2e, prog2->n_tiles, n_work, next_sched_pair(dev), 1);
   } else {
     const unsigned grid = static_cast<unsigned>(prog.n_tiles) * Hq;
     sap_fwd_kernel<D, PARTIAL><<<grid, kFwdThreads, FwdSmem<D>::kTotal, stream>>>(
@@ -408,7 +426,7 @@ int sap_debug_clear_trace(void) {   // zero everything; slots 21 / 53 (atomicMin
   return (int)cudaMemcpyToSymbol(g_sap_trace, h, sizeof(h));
 }
 #endif
-int sap_debug_set_fwd_form(int form) { return g_fwd_form.exchange(form ? 1 : 0); }
+int sap_debug_set_fwd_form(int form) { return g_fwd_form.exchange(form == 1 || form == 2 ? form : 0); }
 int sap_debug_set_bwd_form(int form) { return g_bwd_form.exchange(form ? 1 : 0); }
 int sap_debug_set_bwd_stages(int mask) { return g_bwd_stages.exchange(mask < 0 ? kBwdDefaultStages : (mask & 31)); }
 
@@ -422,10 +440,11 @@ int sap_plan_upload(sap_plan_t* plan) {
   if (pd && pd->uploaded) return pd->device == dev ? SAP_OK : SAP_ERR_PLAN_MISMATCH;   // a plan's mirror lives on one device
   if (!pd) { pd = new PlanDevice(); plan->dev_state = pd; }
   pd->device = dev;
-  if ((rc = upload_program(plan->fwd, pd->fwd)) == SAP_OK && (rc = upload_program(plan->kv, pd->kv)) == SAP_OK)
-    rc = upload_program(plan->kv2, pd->kv2);
+  if ((rc = upload_program(plan->fwd, pd->fwd)) == SAP_OK && (rc = upload_program(plan->kv, pd->kv)) == SAP_OK &&
+      (rc = upload_program(plan->kv2, pd->kv2)) == SAP_OK)
+    rc = upload_program(plan->fwd2, pd->fwd2);
   if (rc != SAP_OK) {  // leave nothing half-uploaded behind: a retry starts from scratch
-    free_program(pd->fwd); free_program(pd->kv); free_program(pd->kv2);
+    free_program(pd->fwd); free_program(pd->kv); free_program(pd->kv2); free_program(pd->fwd2);
     return rc;
   }
   pd->uploaded = true;
@@ -441,6 +460,7 @@ void sap_plan_destroy(sap_plan_t* plan) {
     free_program(pd->fwd);
     free_program(pd->kv);
     free_program(pd->kv2);
+    free_program(pd->fwd2);
     for (auto& cache : pd->ranges)
       for (auto& e : cache) { free_program(e.dev); if (e.ready) cudaEventDestroy(e.ready); }
     if (switched) cudaSetDevice(cur);
@@ -468,8 +488,8 @@ int sap_attn_fwd(const void* q, const void* k, const void* v, const int32_t* cu_
   const PlanDevice* pd = static_cast<const PlanDevice*>(plan->dev_state);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (head_dim == 128)
-    return launch_fwd<128, false>(pd->fwd, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st);
-  return launch_fwd<64, false>(pd->fwd, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st);
+    return launch_fwd<128, false>(pd->fwd, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st, &pd->fwd2);
+  return launch_fwd<64, false>(pd->fwd, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st, &pd->fwd2);
 }
 
 int sap_attn_fwd_partial(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev, sap_plan_t* plan,

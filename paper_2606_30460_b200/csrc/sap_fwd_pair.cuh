@@ -38,11 +38,14 @@ struct FwdPairSmem {
 
 // Work item w of a launch -> (kv-head, Q tile, first q-head of the pair): kv-head-major, tiles longest-first inside a
 // head, the g/2 head pairs of a tile adjacent (CTAs that run side by side share one kv-head's K/V in L2).
+// Two forms of a work item's two 128-row units: head pairs (row_pair = 0: units A, B = q-heads h0, h0 + 1 of one GQA group on
+// the same 128 rows; even Hq/Hkv) and row pairs (row_pair = 1: rows [row0, +128) and [row0 + 128, +128) of ONE q-head, over
+// a 256-row tile program; any Hq/Hkv, used for the odd ones, e.g. MHA).  Either way both units stream the same K/V tiles.
 struct FwdPairWork { int hk, tile_idx, h0; };
-__device__ __forceinline__ FwdPairWork fwd_pair_work(int w, int n_tiles, int g) {
-  const int pairs = g / 2, per_head = n_tiles * pairs;
+__device__ __forceinline__ FwdPairWork fwd_pair_work(int w, int n_tiles, int g, int row_pair) {
+  const int pairs = row_pair ? g : g / 2, per_head = n_tiles * pairs;
   const int hk = w / per_head, rem = w % per_head;
-  return {hk, rem / pairs, hk * g + 2 * (rem % pairs)};
+  return {hk, rem / pairs, hk * g + (row_pair ? 1 : 2) * (rem % pairs)};
 }
 // One slot of the work ring the scheduler thread fills ahead of the other roles: everything they need to start an item
 // without a global load of their own (tile, first segment, iteration count, and the cu_seqlens entries around the tile's
@@ -74,7 +77,7 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
                     const SegDesc* __restrict__ segs, const int32_t* __restrict__ cu, int n_docs,
                     __nv_bfloat16* __restrict__ out, float* __restrict__ out_f32, float* __restrict__ lse,
                     int n_tokens, int n_q_heads, int n_kv_heads, float scale_log2, int n_tiles, int n_work,
-                    int* __restrict__ sched) {
+                    int* __restrict__ sched, int row_pair) {
   using L = FwdPairSmem<D>;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = smem_raw;
@@ -128,7 +131,7 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
           TileDesc td = {0, 0, 0, 0};
           int n_it = 0, e0 = 0, n_cu = 0;
           if (!end) {   // all global loads of the item's metadata happen here, ahead of the roles that use it
-            wk = fwd_pair_work(w, n_tiles, g);
+            wk = fwd_pair_work(w, n_tiles, g, row_pair);
             td = tiles[wk.tile_idx];
             n_it = fwd_tile_iters(td, segs);
             int lo = 0, hi = n_docs;   // e0 = document of row0: cu[e0] <= row0 < cu[hi]
@@ -160,7 +163,8 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
           for (int x = 0; x < 2; ++x)
 #pragma unroll
             for (int b = 0; b < L::kBoxes; ++b)
-              tma_load_2d(sQ + x * L::kTileBytes + b * L::kBoxBytes, &mapQ, (wk.h0 + x) * D + b * 64, td.row0, bar_q_full);
+              tma_load_2d(sQ + x * L::kTileBytes + b * L::kBoxBytes, &mapQ, (wk.h0 + (row_pair ? 0 : x)) * D + b * 64,
+                          td.row0 + (row_pair ? kTile * x : 0), bar_q_full);   // rows past the end of the tensor are zero-filled
           for (int s = td.seg_begin; s < td.seg_end; ++s) {
             const int c_begin = segs[s].t_begin, c_end = segs[s].t_end;
             for (int c0 = c_begin; c0 < c_end; c0 += kTile) {
@@ -279,8 +283,9 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
       if (w >= 0) {
         td.row0 = slot->row0; td.rows = slot->rows; td.seg_begin = slot->seg_begin; td.seg_end = slot->seg_end;
         n_iters = slot->n_iters;
-        t = td.row0 + r;
-        valid = r < td.rows;
+        const int r_unit = (row_pair ? kTile * x : 0) + r;   // row inside the tile (row pairs: unit B = rows 128..255)
+        t = td.row0 + r_unit;
+        valid = r_unit < td.rows;
         const int n_cu = slot->n_cu;
         doc_lo = slot->cu_win[0];   // start of the row's document: the last window entry <= t (cu is non-decreasing)
 #pragma unroll
@@ -299,8 +304,8 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
       if (++ws == 2) { ws = 0; wph ^= 1; }
       if (w < 0) break;
       if (far) doc_lo = doc_start_of(cu, n_docs, t);
-      const FwdPairWork wk = fwd_pair_work(w, n_tiles, g);
-      const int h = wk.h0 + x;
+      const FwdPairWork wk = fwd_pair_work(w, n_tiles, g, row_pair);
+      const int h = wk.h0 + (row_pair ? 0 : x);
       float m_used = -CUDART_INF_F;  // reference max (log2 domain) the running sum and O are scaled by
       float l_run = 0.f;
       int it = 0;

@@ -44,7 +44,7 @@ enum { kRangeItemsQ = 0, kRangeQ = 1, kRangeKv = 2, kRangeKvPair = 3, kRangeItem
 struct PlanDevice {
   bool uploaded = false;
   int device = -1;
-  DevProgram fwd, kv, kv2;
+  DevProgram fwd, kv, kv2, fwd2;
   std::list<RangeProgram> ranges[kRangeKinds];   // most recently used first
 };
 

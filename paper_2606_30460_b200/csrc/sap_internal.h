@@ -12,7 +12,7 @@ constexpr int kTile = 128;  // rows of a Q tile and of a K/V tile
 // One stationary tile of a kernel: a Q tile (fwd, bwd-dQ) or a K/V tile (bwd-dKdV).
 struct TileDesc {
   int32_t row0;       // first token of the tile
-  int32_t rows;       // valid tokens (1..128; 1..256 for the K/V pair-tiles of sap_bwd_pair_kernel)
+  int32_t rows;       // valid tokens (1..128; 1..256 for the K/V pair-tiles of sap_bwd_pair_kernel and the row-pair Q tiles)
   int32_t seg_begin;  // segments [seg_begin, seg_end) of the matching SegDesc array
   int32_t seg_end;
 };
@@ -44,6 +44,7 @@ struct sap_plan {
   std::vector<uint8_t> kind_map;
   int64_t useful_pairs = 0;
   sap::TileProgram fwd;  // Q-stationary: forward and backward-dQ
+  sap::TileProgram fwd2; // Q-stationary, 256-row tiles = two 128-row units of one head (row-pair forward: odd Hq/Hkv, MHA)
   sap::TileProgram kv;   // KV-stationary: backward-dK/dV, 128-key tiles (one CTA per tile)
   sap::TileProgram kv2;  // KV-stationary, 256-key pair-tiles (one CTA pair per tile)
   std::mutex mu;
@@ -53,7 +54,8 @@ struct sap_plan {
 namespace sap {
 // Build a Q-stationary tile program restricted to items [item_begin, item_end).
 // `drop_empty`: leave out tiles that have no work among those items (a rank's launch touches only its own rows).
-void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, TileProgram& out, bool drop_empty = false);
+void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, TileProgram& out, bool drop_empty = false,
+                     int32_t tile_rows = kTile);
 // K/V tiles of kv-chunks [chunk_begin, chunk_end) only (the whole sequence by default).
 // `item_begin..item_end` keeps only segments of those plan items; `drop_empty` leaves out tiles without work.
 void build_kv_program(const sap_plan& p, TileProgram& out, int32_t chunk_begin = 0, int32_t chunk_end = -1, int32_t tile_rows = kTile,

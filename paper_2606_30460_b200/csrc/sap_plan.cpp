@@ -49,7 +49,7 @@ static void order_tiles(TileProgram& out, const std::vector<int64_t>& work, cons
   out.tiles.swap(sorted);
 }
 
-void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, TileProgram& out, bool drop_empty) {
+void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, TileProgram& out, bool drop_empty, int32_t tile_rows) {
   out.tiles.clear();
   out.segs.clear();
   out.streamed_tiles = 0;
@@ -58,8 +58,8 @@ void build_q_program(const sap_plan& p, int32_t item_begin, int32_t item_end, Ti
   std::vector<int32_t> group;
   for (int32_t i = 0; i < p.n_chunks; ++i) {
     const int64_t c_begin = (int64_t)i * n, c_end = c_begin + n;
-    for (int64_t r0 = c_begin; r0 < c_end; r0 += kTile) {
-      const int64_t r1 = std::min<int64_t>(r0 + kTile, c_end);
+    for (int64_t r0 = c_begin; r0 < c_end; r0 += tile_rows) {   // 128 rows; 256 = two 128-row units of the row-pair forward
+      const int64_t r1 = std::min<int64_t>(r0 + tile_rows, c_end);
       TileDesc td;
       td.row0 = (int32_t)r0;
       td.rows = (int32_t)(r1 - r0);
@@ -214,6 +214,7 @@ int sap_plan_create(const int32_t* cu, int32_t n_docs, int32_t n_chunks, sap_pla
     p->useful_pairs += L * (L + 1) / 2;
   }
   build_q_program(*p, 0, (int32_t)p->items.size(), p->fwd);
+  build_q_program(*p, 0, (int32_t)p->items.size(), p->fwd2, false, 2 * kTile);
   build_kv_program(*p, p->kv);
   build_kv_program(*p, p->kv2, 0, -1, 2 * kTile);
   *out = p;
@@ -380,6 +381,7 @@ int32_t sap_debug_tile_program(const sap_plan_t* p, int32_t kind, int32_t a, int
     case 4: if (!items_ok()) return -SAP_ERR_INVALID_ARG; build_q_program(*p, a, b, built, true); break;
     case 5: if (!chunks_ok()) return -SAP_ERR_INVALID_ARG; build_q_program(*p, p->chunk_offsets[a], p->chunk_offsets[b], built, true); break;
     case 6: case 7: if (!chunks_ok()) return -SAP_ERR_INVALID_ARG; build_kv_program(*p, built, a, b, kind == 7 ? 2 * kTile : kTile); break;
+    case 10: prog = &p->fwd2; break;
     case 8: case 9: if (!items_ok()) return -SAP_ERR_INVALID_ARG; build_kv_program(*p, built, 0, -1, kind == 9 ? 2 * kTile : kTile, a, b, true); break;
     default: return -SAP_ERR_INVALID_ARG;
   }

@@ -171,3 +171,21 @@ def test_fwd_persistent_scheduler_many_launches_two_streams():
         for j in range(3):
             assert torch.equal(outs[si][j], ref_out), f"stream {si} buffer {j}: out differs"
             assert torch.equal(lses[si][j], ref_lse), f"stream {si} buffer {j}: lse differs"
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_fwd_row_pair_form_matches_oracle(name):
+    """The row-pair form of the persistent forward (two 128-row halves of a 256-row tile of ONE q-head per work item: what
+    sap_attn_fwd launches for odd Hq/Hkv, e.g. MHA, on long sequences) forced on every small case - one tile, ragged tails,
+    empty and one-token documents, chunk lengths that are not multiples of 256, GQA and MHA, d = 64 and 128 - every element
+    against the oracle."""
+    lens, P, Hq, Hkv, d = CASES[name]
+    w = custom_workload(lens, P, Hq, Hkv, d, name=name)
+    prev = sap.sap_debug_set_fwd_form(2)
+    try:
+        (q, k, v), plan, out, lse = run_fwd(w)
+    finally:
+        sap.sap_debug_set_fwd_form(prev)
+    o_ref, l_ref = oracle.attn_fwd(to_np(q), to_np(k), to_np(v), w.cu_seqlens, w.softmax_scale)
+    check_close(to_np(out), o_ref, f"{name}: out (row pairs)")
+    check_lse(to_np(lse).T, l_ref, f"{name}: lse (row pairs)")

@@ -59,7 +59,7 @@ def test_every_visible_pair_is_covered_exactly_once(seed):
     all_items = list(range(n_items))
     want_all, _ = visible_matrix(cu, items, all_items)
     assert want_all.max() <= 1                                   # items are disjoint (oracle pin P11 on the library's plan)
-    for kind in (0, 1, 2):                                       # the programs sap_attn_fwd / sap_attn_bwd walk
+    for kind in (0, 1, 2, 10):                                   # the programs sap_attn_fwd / sap_attn_bwd walk (10: 256-row Q tiles)
         got, _ = replay(plan, cu, kind)
         assert np.array_equal(got, want_all), (kind, cu, P)
     a = int(rng.integers(0, n_items)); b = int(rng.integers(a, n_items + 1))
