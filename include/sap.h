@@ -159,8 +159,8 @@ size_t sap_workspace_bytes(const sap_plan_t* plan, int n_q_heads, int n_kv_heads
  * q,k,v,cu_seqlens_dev: device, read.  out: device bf16 [N,Hq,d], written.  lse: device fp32 [Hq,N], written.
  * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Asynchronous.
  * With an even Hq/Hkv the launch is persistent (one CTA per SM; work items = (Q tile, pair of q-heads of a group) taken
- * in order off a device counter).  The counters come from a per-device pool of 64 pairs that launches take round-robin
- * and that each launch leaves zeroed: calls may overlap on different streams as long as fewer than 64 forward launches
+ * in order off a device counter).  The counters come from a per-device pool of 256 pairs that launches take round-robin
+ * and that each launch leaves zeroed: calls may overlap on different streams as long as fewer than 256 forward launches
  * of one process are in flight on one device at the same time. */
 int sap_attn_fwd(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev,
                  sap_plan_t* plan, int64_t n_tokens, void* out, float* lse,

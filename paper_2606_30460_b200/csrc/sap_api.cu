@@ -73,7 +73,7 @@ static cudaError_t set_kernel_attributes() {
 // Per-device state of the persistent kernels: the SM count and a pool of {next, done} counter pairs (zero between
 // launches: the last CTA of a launch re-arms its pair).  Launches take the pairs round-robin, so kernels that run
 // concurrently on different streams do not share one unless more than kSchedSlots are in flight at once.
-constexpr int kSchedSlots = 64;
+constexpr int kSchedSlots = 256;
 struct DeviceSched { int n_sms = 0; int* pool = nullptr; std::atomic<unsigned> seq{0}; };
 static DeviceSched g_sched[64];
 
@@ -342,6 +342,7 @@ static int get_range_program(sap_plan_t* plan, int kind, int32_t a, int32_t b, c
       case kRangeItemsQ: build_q_program(*plan, a, b, e.host); break;                                               // partial forward, every row
       case kRangeItemsQDrop: build_q_program(*plan, a, b, e.host, true); break;                                     // ... touched Q tiles only
       case kRangeQ: build_q_program(*plan, plan->chunk_offsets[a], plan->chunk_offsets[b], e.host, true); break;    // q-chunks
+      case kRangeQ2: build_q_program(*plan, plan->chunk_offsets[a], plan->chunk_offsets[b], e.host, true, 2 * kTile); break;   // ... in 256-row tiles
       case kRangeKv: case kRangeKvPair: build_kv_program(*plan, e.host, a, b, kv_rows); break;                      // kv-chunks
       default: build_kv_program(*plan, e.host, 0, -1, kv_rows, a, b, true); break;                                  // items, KV-stationary
     }
@@ -582,9 +583,12 @@ int sap_attn_fwd_chunks(const void* q, const void* k, const void* v, const int32
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   DevProgram prog;
   if ((rc = get_range_program(plan, kRangeQ, q_chunk_begin, q_chunk_end, st, &prog)) != SAP_OK) return rc;
+  DevProgram prog2;   // odd Hq/Hkv (MHA): the row-pair form needs the same rows in 256-row tiles
+  const bool odd = (n_q_heads / n_kv_heads) % 2 != 0;
+  if (odd && (rc = get_range_program(plan, kRangeQ2, q_chunk_begin, q_chunk_end, st, &prog2)) != SAP_OK) return rc;
   if (head_dim == 128)
-    return launch_fwd<128, false>(prog, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st);
-  return launch_fwd<64, false>(prog, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st);
+    return launch_fwd<128, false>(prog, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st, odd ? &prog2 : nullptr);
+  return launch_fwd<64, false>(prog, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st, odd ? &prog2 : nullptr);
 }
 
 int sap_attn_bwd_begin(const void* dout, const void* out, sap_plan_t* plan, int64_t n_tokens, int32_t q_chunk_begin,

@@ -37,7 +37,7 @@ struct RangeProgram {
   cudaEvent_t ready = nullptr; // recorded behind the upload: other streams wait on it
   cudaStream_t stream = nullptr;
 };
-enum { kRangeItemsQ = 0, kRangeQ = 1, kRangeKv = 2, kRangeKvPair = 3, kRangeItemsKv = 4, kRangeItemsKvPair = 5, kRangeItemsQDrop = 6, kRangeKinds = 7 };
+enum { kRangeItemsQ = 0, kRangeQ = 1, kRangeKv = 2, kRangeKvPair = 3, kRangeItemsKv = 4, kRangeItemsKvPair = 5, kRangeItemsQDrop = 6, kRangeQ2 = 7, kRangeKinds = 8 };
 
 // Device copies owned by a plan (freed by sap_plan_destroy).  A plan's mirror lives on ONE device (the current
 // device of the first upload); calls with another current device return SAP_ERR_PLAN_MISMATCH.

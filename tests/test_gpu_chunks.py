@@ -87,3 +87,29 @@ def test_chunk_api_rejects_bad_ranges_and_unaligned_chunks():
     sap.sap_attn_fwd_chunks(q, k, v, cu, plan, 1, 2, out2, lse2)      # the forward has no alignment requirement
     torch.cuda.synchronize()
     assert torch.equal(out2[200:400], out[200:400]) and bool(torch.isnan(out2[:200]).all()) and bool(torch.isnan(out2[400:]).all())
+
+
+@pytest.mark.parametrize("lens,P,Hq,Hkv,d", [
+    ([2048], 8, 2, 2, 64),                        # MHA: chunks of 256 rows = one row-pair tile each
+    ([700, 1100, 504], 6, 3, 1, 128),             # group of 3, chunks of 384 rows: a full pair tile and a half one per chunk
+])
+def test_rank_by_rank_forward_on_row_pairs(lens, P, Hq, Hkv, d):
+    """The per-rank forward of odd Hq/Hkv in the row-pair form (forced: these shapes are below its size threshold): the P
+    launches write only their own rows and together equal the oracle, every element."""
+    w = custom_workload(lens, P, Hq, Hkv, d)
+    q, k, v = make_qkv(w, device="cuda", with_dout=False)
+    plan = sap.sap_plan(w.cu_seqlens, P)
+    cu = plan.cu_seqlens_dev("cuda")
+    out = torch.full_like(q, float("nan")); lse = torch.full((Hq, w.n_tokens), float("nan"), device="cuda")
+    n = w.n_tokens // P
+    prev = sap.sap_debug_set_fwd_form(2)
+    try:
+        for c in reversed(range(P)):
+            sap.sap_attn_fwd_chunks(q, k, v, cu, plan, c, c + 1, out, lse, softmax_scale=w.softmax_scale)
+            torch.cuda.synchronize()
+            assert bool(torch.isnan(out[: c * n]).all()), "a rank wrote rows of an earlier chunk"
+    finally:
+        sap.sap_debug_set_fwd_form(prev)
+    o_ref, l_ref = oracle.attn_fwd(to_np(q), to_np(k), to_np(v), w.cu_seqlens, w.softmax_scale)
+    check_close(to_np(out), o_ref, "out, per-rank row pairs")
+    check_lse(to_np(lse).T, l_ref, "lse, per-rank row pairs")

@@ -150,7 +150,7 @@ def test_fwd_rejects_bad_arguments():
 
 def test_fwd_persistent_scheduler_many_launches_two_streams():
     """The persistent forward takes its work items off {next, done} counter pairs that the last CTA of a launch re-arms
-    (sap_api.cu: kSchedSlots = 64 pairs per device, handed out round-robin).  150 launches - every pair reused - issued
+    (sap_api.cu: kSchedSlots = 256 pairs per device, handed out round-robin).  600 launches - every pair reused - issued
     alternately on two streams, so launches overlap: every one must reproduce the first result bit for bit (the
     forward has no atomics on its outputs), with more work items than SMs and a ragged last tile."""
     w = custom_workload([3000, 1500, 2500 + 77, 1115], 4, 8, 2, 128, name="sched")
@@ -162,7 +162,7 @@ def test_fwd_persistent_scheduler_many_launches_two_streams():
     streams = [torch.cuda.Stream(), torch.cuda.Stream()]
     outs = [[torch.empty_like(ref_out) for _ in range(3)] for _ in streams]
     lses = [[torch.empty_like(ref_lse) for _ in range(3)] for _ in streams]
-    for it in range(75):
+    for it in range(300):
         for si, st in enumerate(streams):
             o, l = outs[si][it % 3], lses[si][it % 3]
             sap.sap_attn_fwd(q, k, v, cu, plan, out=o, lse=l, softmax_scale=w.softmax_scale, stream=st)
