@@ -52,7 +52,8 @@ enum {
   SAP_ERR_WRONG_ARCH = 6,         /* current device is not compute capability 10.x                    */
   SAP_ERR_CUDA = 7,               /* a CUDA runtime/driver call failed; see sap_last_cuda_error()     */
   SAP_ERR_NO_DEVICE = 8,          /* no CUDA device / driver available                                */
-  SAP_ERR_PLAN_MISMATCH = 9       /* n_tokens != the plan's token count, or the plan's mirror is on another device */
+  SAP_ERR_PLAN_MISMATCH = 9,      /* n_tokens != the plan's token count, or the plan's mirror is on another device */
+  SAP_ERR_STATIC_LIMIT = 10       /* sap_attn_bwd_static: the problem does not fit the library's built-in scratch memory */
 };
 
 /* ---- plan (host-side JIT planner; §3.2 Step 1, :106-:108) ------------------------- */
@@ -199,6 +200,37 @@ int sap_attn_bwd(const void* dout, const void* q, const void* k, const void* v, 
                  void* dq, void* dk, void* dv,
                  int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
                  void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---- backward without allocation --------------------------------------------------------------------------------
+ * The same backward pass as sap_attn_bwd (same kernels, same arguments and layouts, same results) for callers that
+ * have no way to obtain device memory at the point where they need the gradients: code that runs under a framework
+ * whose memory pool is the only permitted allocator and is not reachable from there, a callback or plug-in that is
+ * handed tensors but no allocator, a real-time or already memory-budgeted process in which cudaMalloc (a device-wide
+ * synchronisation that can also fail late) is ruled out after start-up.  sap_attn_bwd asks such a caller for two
+ * things it cannot give: a workspace buffer, and - on the first use of a plan - sap_plan_upload, which calls
+ * cudaMalloc.  This entry point needs neither.  The tile program and the workspace (D and the fp32 dQ accumulator)
+ * live in a fixed array that is part of the library image on the device: SAP_STATIC_WORKSPACE_BYTES + 256 KiB per GPU
+ * that loads the library, held until the process exits whether or not this function is ever called.
+ *   - The call itself runs no cudaMalloc, cudaFree, or any other allocating routine, and never uploads the plan's
+ *     device mirror; the tile program is copied from the plan's host memory on cuda_stream at every call.
+ *   - Limit: sap_workspace_bytes(plan, Hq, Hkv, d, SAP_PASS_BWD) <= SAP_STATIC_WORKSPACE_BYTES, i.e. about
+ *     N * Hq * (d + 1) * 4 bytes <= 16 MiB (4096 tokens x 8 q-heads at d = 128), and a tile program of at most 256 KiB
+ *     (not reached by plans within the first limit unless they hold thousands of documents).  Anything larger returns
+ *     SAP_ERR_STATIC_LIMIT before the device is touched; use sap_attn_bwd with your own workspace then.
+ *   - The first call on each device also does that device's one-time set-up (kernel attributes, looking up the
+ *     array's device address, and the driver loading the kernels).  Make that first call before any stream capture.
+ *   - All calls of a process on one device share the one array.  It keeps what the previous call left; each call
+ *     rewrites the program and D and clears the accumulator on cuda_stream before its kernels run.  Calls on the same
+ *     stream are therefore safe back to back; two calls that can overlap on the GPU (different streams without an
+ *     ordering between them, or different host threads) race on the array and give wrong gradients with no error.
+ *     sap_attn_bwd with separate workspaces is the form for concurrent use.
+ *   - Returns SAP_ERR_UNSUPPORTED while a non-default sap_debug_set_bwd_stages mask is in force.  Otherwise errors and
+ *     asynchrony as sap_attn_bwd; dq, dk, dv are outputs the caller owns. */
+#define SAP_STATIC_WORKSPACE_BYTES ((size_t)16 << 20)
+int sap_attn_bwd_static(const void* dout, const void* q, const void* k, const void* v, const void* out,
+                        const float* lse, const int32_t* cu_seqlens_dev, sap_plan_t* plan, int64_t n_tokens,
+                        void* dq, void* dk, void* dv,
+                        int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale, void* cuda_stream);
 
 /* ---- per-rank launches ------------------------------------------------------------------
  * The same kernels restricted to the chunks one rank owns (rank i holds Q_i, K_i, V_i).  Token indices

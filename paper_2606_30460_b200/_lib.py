@@ -47,6 +47,8 @@ SIGNATURES = {
                                      ctypes.c_int, ctypes.c_int64, ctypes.c_int64, vp]),
     "sap_attn_bwd": (ctypes.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, ctypes.c_int64, vp, vp, vp, ctypes.c_int, ctypes.c_int,
                                     ctypes.c_int, ctypes.c_float, vp, ctypes.c_size_t, vp]),
+    "sap_attn_bwd_static": (ctypes.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, ctypes.c_int64, vp, vp, vp, ctypes.c_int, ctypes.c_int,
+                                           ctypes.c_int, ctypes.c_float, vp]),
     "sap_attn_fwd_chunks": (ctypes.c_int, [vp, vp, vp, vp, vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, vp, vp, ctypes.c_int,
                                            ctypes.c_int, ctypes.c_int, ctypes.c_float, vp]),
     "sap_attn_bwd_begin": (ctypes.c_int, [vp, vp, vp, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.c_int, ctypes.c_int,

@@ -248,6 +248,22 @@ def sap_attn_bwd(dout, q, k, v, out, lse, cu_seqlens_dev, plan: Plan, softmax_sc
     return dq, dk, dv
 
 
+def sap_attn_bwd_static(dout, q, k, v, out, lse, cu_seqlens_dev, plan: Plan, dq, dk, dv, softmax_scale: Optional[float] = None,
+                        stream=None):
+    """sap_attn_bwd for callers that cannot allocate device memory where they need the gradients (a plug-in that is
+    handed tensors but no allocator, code running where only a framework's pool may allocate): the workspace and the
+    plan's tile program sit in a fixed array inside the library, so this binding allocates nothing either - dq, dk, dv
+    must be passed in.  Problems whose workspace exceeds 16 MiB raise SapError (status 10).  One array per GPU is shared
+    by all calls: keep them on one stream, or otherwise ordered; overlapping calls corrupt each other.  See sap.h."""
+    _require_cuda_bf16(dout, q, k, v, out, dq, dk, dv)
+    N, Hq, Hkv, d = _dims(q, k)
+    scale = float(d) ** -0.5 if softmax_scale is None else float(softmax_scale)
+    _check(_lib.lib().sap_attn_bwd_static(_ptr(dout), _ptr(q), _ptr(k), _ptr(v), _ptr(out), _ptr(lse), _ptr(cu_seqlens_dev),
+                                          plan.handle, N, _ptr(dq), _ptr(dk), _ptr(dv), Hq, Hkv, d, scale, _stream(stream)),
+           "sap_attn_bwd_static")
+    return dq, dk, dv
+
+
 def sap_launch_count() -> int:
     return int(_lib.lib().sap_launch_count())
 

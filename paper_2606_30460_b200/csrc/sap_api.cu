@@ -681,3 +681,97 @@ int sap_axpy(void* dst, int dst_is_bf16, const void* src, int src_is_bf16, int64
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// sap_attn_bwd_static (include/sap.h): the backward pass for callers that must not allocate device memory.
+//
+// sap_attn_bwd needs two pieces of device memory besides its tensors: the plan's tile programs (sap_plan_upload:
+// cudaMalloc + a synchronous copy) and the caller's workspace (D and the fp32 dQ accumulator).  Here both live in one
+// file-scope device array that comes with the library image: nobody allocates it and nobody frees it.
+//
+//   g_static_scratch = [ tile program: tiles | segs    (kStaticProgramBytes)
+//                      | workspace: D [Hq,N] fp32 | dQ accumulator [N,Hq,d] fp32   (SAP_STATIC_WORKSPACE_BYTES) ]
+//
+// In host code the identifier g_static_scratch is only the host-side handle of the symbol - it is not a device
+// address and must never reach a kernel or a memcpy as one.  The device address is looked up once per device with
+// cudaGetSymbolAddress (below, with that device current) and everything on the host works from that pointer.
+// ---------------------------------------------------------------------------------------------------------------------
+namespace sap {
+
+constexpr size_t kStaticProgramBytes = size_t(256) << 10;   // far more than any plan whose workspace fits below needs
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticProgramBytes + SAP_STATIC_WORKSPACE_BYTES];
+
+static unsigned char* g_static_base[64];   // device address of g_static_scratch per device; null = not set up yet
+static std::mutex g_static_mu;
+
+// Set-up of the current device for sap_attn_bwd_static, on its first call there: architecture check, the kernels'
+// shared-memory opt-ins, the address of the scratch array.  Unlike ensure_device it allocates nothing (that one also
+// creates the forward's counter pool with cudaMalloc), so the two are kept apart.
+static int ensure_device_static(unsigned char** base) {
+  int dev = 0;
+  SAP_CUDA_CHECK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return SAP_ERR_UNSUPPORTED;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_base[dev]) {
+    int major = 0;
+    SAP_CUDA_CHECK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return SAP_ERR_WRONG_ARCH;
+    const cudaFuncAttribute a = cudaFuncAttributeMaxDynamicSharedMemorySize;
+    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_fused_kernel<64>, a, FusedSmem<64>::kTotal));
+    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_fused_kernel<128>, a, FusedSmem<128>::kTotal));
+    SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_pair_kernel, a, PairSmem::kTotal));
+    void* p = nullptr;
+    SAP_CUDA_CHECK(cudaGetSymbolAddress(&p, g_static_scratch));
+    if (!p) { g_last_cuda_error = static_cast<int>(cudaErrorInvalidSymbol); return SAP_ERR_CUDA; }
+    g_static_base[dev] = static_cast<unsigned char*>(p);
+  }
+  *base = g_static_base[dev];
+  return SAP_OK;
+}
+
+}  // namespace sap
+
+extern "C" int sap_attn_bwd_static(const void* dout, const void* q, const void* k, const void* v, const void* out,
+                                   const float* lse, const int32_t* cu_seqlens_dev, sap_plan_t* plan, int64_t n_tokens,
+                                   void* dq, void* dk, void* dv, int n_q_heads, int n_kv_heads, int head_dim,
+                                   float softmax_scale, void* cuda_stream) {
+  if (!dout || !q || !k || !v || !out || !lse || !cu_seqlens_dev || !dq || !dk || !dv || !plan) return SAP_ERR_INVALID_ARG;
+  if (n_q_heads < 1 || n_kv_heads < 1 || !(softmax_scale > 0.f)) return SAP_ERR_INVALID_ARG;
+  if ((head_dim != 64 && head_dim != 128) || n_q_heads % n_kv_heads != 0) return SAP_ERR_UNSUPPORTED;
+  if (n_tokens != plan->n_tokens) return SAP_ERR_PLAN_MISMATCH;
+  if (!aligned16(dout) || !aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out) || !aligned16(dq) ||
+      !aligned16(dk) || !aligned16(dv))
+    return SAP_ERR_UNSUPPORTED;
+  if (g_bwd_stages.load() != kBwdDefaultStages) return SAP_ERR_UNSUPPORTED;   // the diagnostic split forms walk other programs
+  // the limits, checked before anything touches the device
+  const TileProgram& host = use_pair_kernel(head_dim) ? plan->kv2 : plan->kv;   // the program the main kernel walks
+  const size_t tiles_bytes = align256(host.tiles.size() * sizeof(TileDesc));
+  const size_t segs_bytes = (host.segs.size() + 1) * sizeof(SegDesc);            // the kernels read one descriptor ahead
+  if (tiles_bytes + segs_bytes > kStaticProgramBytes) return SAP_ERR_STATIC_LIMIT;
+  if (sap_workspace_bytes(plan, n_q_heads, n_kv_heads, head_dim, SAP_PASS_BWD) > SAP_STATIC_WORKSPACE_BYTES) return SAP_ERR_STATIC_LIMIT;
+  unsigned char* base = nullptr;
+  int rc = ensure_device_static(&base);
+  if (rc != SAP_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  // This call's tile program goes into the scratch array on the caller's stream, in front of the kernels that read it.
+  // The source is the plan's host copy, which lives as long as the plan.
+  PlanDevice pd;
+  DevProgram prog;
+  prog.tiles = reinterpret_cast<TileDesc*>(base);
+  prog.segs = reinterpret_cast<SegDesc*>(base + tiles_bytes);
+  prog.n_tiles = static_cast<int32_t>(host.tiles.size());
+  if (!host.tiles.empty())
+    SAP_CUDA_CHECK(cudaMemcpyAsync(prog.tiles, host.tiles.data(), host.tiles.size() * sizeof(TileDesc), cudaMemcpyHostToDevice, st));
+  if (!host.segs.empty())
+    SAP_CUDA_CHECK(cudaMemcpyAsync(prog.segs, host.segs.data(), host.segs.size() * sizeof(SegDesc), cudaMemcpyHostToDevice, st));
+  pd.kv = pd.kv2 = prog;     // launch_bwd_main reads the one that matches the kernel it picks
+  // The workspace half: D is overwritten in full by the pre-pass; the accumulator still holds the previous call's sums
+  // and is cleared by launch_bwd (cudaMemsetAsync on the stream) in front of the main kernel.
+  float* dsum = reinterpret_cast<float*>(base + kStaticProgramBytes);
+  float* dq_acc = reinterpret_cast<float*>(base + kStaticProgramBytes + align256(static_cast<size_t>(plan->n_tokens) * n_q_heads * sizeof(float)));
+  if (head_dim == 128)
+    return launch_bwd<128>(&pd, dout, q, k, v, out, lse, cu_seqlens_dev, plan, dq, dk, dv, n_q_heads, n_kv_heads,
+                           softmax_scale, dsum, dq_acc, st);
+  return launch_bwd<64>(&pd, dout, q, k, v, out, lse, cu_seqlens_dev, plan, dq, dk, dv, n_q_heads, n_kv_heads,
+                        softmax_scale, dsum, dq_acc, st);
+}

@@ -405,6 +405,7 @@ const char* sap_strerror(int status) {
     case SAP_ERR_CUDA: return "CUDA error (see sap_last_cuda_error)";
     case SAP_ERR_NO_DEVICE: return "no CUDA device";
     case SAP_ERR_PLAN_MISMATCH: return "plan mismatch (n_tokens differs from the plan's, or the plan lives on another device)";
+    case SAP_ERR_STATIC_LIMIT: return "problem too large for the built-in scratch memory of sap_attn_bwd_static (SAP_STATIC_WORKSPACE_BYTES)";
     default: return "unknown status";
   }
 }

@@ -34,7 +34,7 @@ def test_argument_errors_come_before_device_errors():
     assert L.sap_attn_fwd(DUMMY, DUMMY, DUMMY, DUMMY, plan.handle, 2048, DUMMY, DUMMY, 4, 4, 64, 0.0, None, 0, None) == 1     # scale
     assert L.sap_axpy(DUMMY, 0, DUMMY, 0, 12, 1.0, 1, None) == 4    # n_elems % 8
     assert L.sap_axpy(None, 0, DUMMY, 0, 16, 1.0, 1, None) == 1
-    for code in range(10):
+    for code in range(11):
         assert L.sap_strerror(code) != b"unknown status"
 
 
