@@ -165,6 +165,15 @@ class ShardView:
         return self._t.data_ptr() - self._row0 * self._t.stride(0) * self._t.element_size()
 
 
+def shard_view_ok(n: int, head_dim: int = 0, backward: bool = False) -> bool:
+    """May shards of n rows be handed to the kernels as ShardViews?  (sap.h, shard-pointer contract.)  The kernels move
+    whole tiles that start on multiples of the tile length - 128 rows; 256 keys for the head_dim-128 backward, which
+    runs on CTA pairs - so a shard boundary inside a tile makes a box reach into the neighbouring shard, outside a
+    shard-sized allocation."""
+    tile = 256 if (backward and head_dim == 128) else 128
+    return n > 0 and n % tile == 0
+
+
 def _max_inflight(code_lists, tensor_kinds):
     """largest number of same-kind RECVs one rank has in one stage: the 'fixed multiple' of a shard the staging area
     needs (PAPER.md:140)"""
@@ -199,7 +208,7 @@ class LocalExecutor:
         self.items = plan.items
         # K/V tiles of the per-item backward are 256 keys (head_dim 128) or 128 keys wide from token 0: a rank's shard-sized
         # dK / dV buffer holds whole tiles only if the chunk length is a multiple of that
-        assert self.n % (256 if head_dim == 128 else 128) == 0, "chunk length must be a multiple of the K/V tile"
+        assert shard_view_ok(self.n, head_dim, backward=True), "chunk length must be a multiple of the K/V tile"
         self.fwd_codes = [plan.codegen(self.slots, r) for r in range(self.P)]
         self.bwd_codes = [plan.codegen(self.slots, r, backward=True) for r in range(self.P)]
         n, Hq, Hkv, d, P = self.n, n_q_heads, n_kv_heads, head_dim, self.P

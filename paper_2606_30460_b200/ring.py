@@ -87,26 +87,44 @@ def cuda_fns(q_shard, cu_seqlens_dev, plan: Plan, rank: int, softmax_scale: Opti
     executor.ShardView (base pointer moved back by the shard's first row) and the forward `computing` entry
     sap_attn_fwd_items touches only the Q tiles of the item, so a rank holds its own Q rows, the K/V shard in flight
     and one partial result: O(N/P) memory and work per item (only the per-row LSE buffer, 4 bytes per row and head,
-    is full length: the library's [Hq, N] layout)."""
+    is full length: the library's [Hq, N] layout).
+
+    That holds when the shard length n = N/P is a multiple of the 128-row tile (sap.h, shard-pointer contract).  The
+    kernels move whole 128-row boxes that start on multiples of 128, so with any other n a box of the first or last
+    tile of a shard reaches rows of the neighbouring shard - memory a shard-sized buffer does not have.  Then the
+    callables fall back to zero-filled full-length buffers with the shard copied into its rows (O(N) memory, same
+    result: rows outside the shard are masked by the item's row and key ranges)."""
     import torch
     from . import api
-    from .executor import ShardView
+    from .executor import ShardView, shard_view_ok
 
     n, Hq, d = q_shard.shape
     N = plan.n_tokens
     dev = q_shard.device
     lo, hi = rank * n, (rank + 1) * n
-    qg = ShardView(q_shard.contiguous(), lo, N)
     lse_full = torch.empty((Hq, N), dtype=torch.float32, device=dev)
+    by_view = shard_view_ok(n)
+
+    def place(shard, row0):
+        """the tensor the kernels see: a view of the shard, or a full-length copy when views are not safe"""
+        if by_view:
+            return ShardView(shard.contiguous(), row0, N)
+        full = torch.zeros((N,) + tuple(shard.shape[1:]), dtype=shard.dtype, device=dev)
+        full[row0:row0 + shard.shape[0]] = shard
+        return full
+
+    qg = place(q_shard, lo)
 
     def partial_fn(item, k_shard, v_shard):
         j = int(plan.items[item, 1])
         Hkv = k_shard.shape[1]
         o = torch.zeros((n, Hq, d), dtype=torch.float32, device=dev)   # Q tiles the item does not touch: the (0, -inf) identity
         lse_full[:, lo:hi] = float("-inf")
-        api.sap_attn_fwd_items(qg, ShardView(k_shard.contiguous(), j * n, N), ShardView(v_shard.contiguous(), j * n, N),
-                               cu_seqlens_dev, plan, item, item + 1, ShardView(o, lo, N), lse_full, Hq, Hkv, d,
-                               softmax_scale=softmax_scale)
+        og = place(o, lo)
+        api.sap_attn_fwd_items(qg, place(k_shard, j * n), place(v_shard, j * n), cu_seqlens_dev, plan, item, item + 1, og,
+                               lse_full, Hq, Hkv, d, softmax_scale=softmax_scale)
+        if not by_view:
+            o = og[lo:hi].contiguous()
         return o, lse_full[:, lo:hi].contiguous()
 
     def merge_fn(o_a, lse_a, o_b, lse_b):

@@ -14,9 +14,11 @@ from parity import check_close, check_lse, to_np
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("P", [1, 4])
-def test_rank_by_rank_partials_equal_fused(P):
-    w = custom_workload([700, 1100, 248], P, 4, 2, 128)
+# P = 5 over 2050 tokens: shards of 410 rows, not a multiple of the 128-row tile - the callables must then hand the kernels
+# full-length buffers (sap.h, shard-pointer contract), since a tile's box would leave a shard-sized allocation
+@pytest.mark.parametrize("P,lens", [(1, [700, 1100, 248]), (4, [700, 1100, 248]), (5, [700, 1100, 250])])
+def test_rank_by_rank_partials_equal_fused(P, lens):
+    w = custom_workload(lens, P, 4, 2, 128)
     q, k, v = make_qkv(w, device="cuda", with_dout=False)
     plan = sap.sap_plan(w.cu_seqlens, P)
     cu = plan.cu_seqlens_dev("cuda")
