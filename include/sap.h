@@ -20,6 +20,12 @@
  *     programs of the partial / per-rank / per-item calls, built on first use of a range and uploaded on
  *     the caller's stream) and frees it in sap_plan_destroy.  Only sap_plan_upload and sap_plan_destroy
  *     synchronise the device; every other call is asynchronous on its stream.
+ *   - Range-restricted programs are cached with the plan, 64 per kind of call; beyond that the least recently used
+ *     one is freed, stream-ordered behind the last kernels that read it on every stream that used it.  Building one
+ *     allocates (cudaMallocAsync) and copies from pageable host memory, so the FIRST use of a range (or the first
+ *     after its eviction) cannot be recorded into a CUDA graph: during stream capture such a call returns
+ *     SAP_ERR_UNSUPPORTED and leaves the capture intact - make the call once outside capture first.  A program a
+ *     graph has recorded a launch on is kept until sap_plan_destroy.
  *   - A plan's device mirror lives on one device (the current device of its first upload); every attention call takes
  *     the caller's token count n_tokens and fails with SAP_ERR_PLAN_MISMATCH when it differs from the plan's (the kernels
  *     index the tensors by the plan's token ranges) or when the current device is another one.
@@ -160,9 +166,13 @@ size_t sap_workspace_bytes(const sap_plan_t* plan, int n_q_heads, int n_kv_heads
  * q,k,v,cu_seqlens_dev: device, read.  out: device bf16 [N,Hq,d], written.  lse: device fp32 [Hq,N], written.
  * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Asynchronous.
  * With an even Hq/Hkv the launch is persistent (one CTA per SM; work items = (Q tile, pair of q-heads of a group) taken
- * in order off a device counter).  The counters come from a per-device pool of 256 pairs that launches take round-robin
- * and that each launch leaves zeroed: calls may overlap on different streams as long as fewer than 256 forward launches
- * of one process are in flight on one device at the same time. */
+ * in order off a device counter).  Each launch needs a counter pair of its own while it runs.  The pairs come from two
+ * per-device pools of 4096 that launches take round-robin and leave zeroed: one pool for ordinary launches, one for
+ * launches recorded during stream capture (a captured launch keeps its pair for the life of the graph, so graph replays
+ * never meet ordinary launches on a pair).  Calls may therefore overlap freely on different streams and with graph
+ * replays, within two limits: fewer than 4096 forward launches of one process in flight on one device at a time, and
+ * at most 4096 forward launches captured into graphs that can run concurrently with each other.  A kernel that finds
+ * its pair was shared traps (the launch fails with a CUDA error) instead of returning wrong output. */
 int sap_attn_fwd(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev,
                  sap_plan_t* plan, int64_t n_tokens, void* out, float* lse,
                  int n_q_heads, int n_kv_heads, int head_dim, float softmax_scale,
@@ -278,7 +288,14 @@ int sap_attn_bwd_end(sap_plan_t* plan, int64_t n_tokens, int32_t q_chunk_begin, 
  * intersect the items' row ranges are computed and written (rows of a touched tile without a visible key among the items
  * get out = 0, lse = -inf); rows of other tiles are left alone.  With tensors addressed through shard-sized buffers
  * (base pointer moved back by the shard's first row) a rank therefore needs memory for one shard of q / out and one of
- * k / v, not for the sequence. */
+ * k / v, not for the sequence.
+ * Shard-pointer contract (both items entry points): the library checks pointers, not what lies behind them.  The
+ * kernels move whole tiles with TMA - 128-row boxes that start on multiples of 128 (q, k, v, dout), 256 keys per K/V
+ * pair-tile in the head_dim-128 backward - and a box is read in full even where the mask then drops its rows.  A
+ * buffer that holds only rows [r0, r0 + n) of a tensor (pointer = buffer - r0 * H * d elements) is therefore legal
+ * only if r0 and n are multiples of 128 (256 for k / v / dk / dv of the head_dim-128 backward); with any other shard
+ * length pass full-length tensors (rows outside the shard may hold anything finite).  executor.shard_view_ok is the
+ * same rule on the Python side; ring.cuda_fns and executor.LocalExecutor apply it. */
 int sap_attn_fwd_items(const void* q, const void* k, const void* v, const int32_t* cu_seqlens_dev,
                        sap_plan_t* plan, int64_t n_tokens, int32_t item_begin, int32_t item_end,
                        float* out_f32, float* lse,
@@ -295,7 +312,6 @@ int sap_attn_bwd_items(const void* dout, const void* q, const void* k, const voi
 int sap_axpy(void* dst, int dst_is_bf16, const void* src, int src_is_bf16, int64_t n_elems, float alpha, int accumulate,
              void* cuda_stream);
 
-/* ---- diagnostics ---------------------------------------------------------------------------- */
 /* ---- stitched allocation: the data plane of real ranks ------------------------------ */
 /* One device virtual address range of n_chunks * chunk_bytes bytes whose chunk c is physical memory of device
  * device_of_chunk[c], readable and writable by every device in access_devices - the layout that lets a rank's launch
@@ -326,6 +342,7 @@ int sap_stitched_create_local(int32_t n_chunks, size_t chunk_bytes, int device, 
 int sap_stitched_export_fd(const sap_stitched_t* s, int32_t chunk, int* fd);
 int sap_stitched_import_fd(sap_stitched_t* s, int32_t chunk, int fd);
 
+/* ---- diagnostics ---------------------------------------------------------------------------- */
 const char* sap_strerror(int status);
 int sap_last_cuda_error(void);      /* the cudaError_t / CUresult of the last SAP_ERR_CUDA on this thread */
 /* Number of kernels the library has launched in this process (all streams); for launch accounting. */

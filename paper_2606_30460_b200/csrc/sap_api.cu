@@ -70,14 +70,26 @@ static cudaError_t set_kernel_attributes() {
   return cudaSuccess;
 }
 
-// Per-device state of the persistent kernels: the SM count and a pool of {next, done} counter pairs (zero between
-// launches: the last CTA of a launch re-arms its pair).  Launches take the pairs round-robin, so kernels that run
-// concurrently on different streams do not share one unless more than kSchedSlots are in flight at once.
-constexpr int kSchedSlots = 256;
-struct DeviceSched { int n_sms = 0; int* pool = nullptr; std::atomic<unsigned> seq{0}; };
+// Per-device state of the persistent kernels: the SM count and two pools of {next, done} counter pairs (zero between
+// launches: the last CTA of a launch re-arms its pair).  A pair must serve one launch at a time.
+//   eager pool   : launches outside stream capture take its pairs round-robin, so two of them hold the same pair only
+//                  if kSchedSlots forward launches are in flight on the device at once.
+//   capture pool : a launch recorded into a CUDA graph keeps its pair for the life of the graph and runs at replay
+//                  time, when the host cannot pick one.  Such launches draw from a pool of their own, so a replay
+//                  never meets an eager launch on its pair; two graphs share a pair only once more than kSchedSlots
+//                  forward launches have been captured in the process (round-robin again).
+// The kernel traps if it finds that its pair was shared (sap_fwd_pair.cuh, last lines).
+constexpr int kSchedSlots = 4096;
+struct DeviceSched { int n_sms = 0; int* pool = nullptr; std::atomic<unsigned> seq{0}, seq_capture{0}; };
 static DeviceSched g_sched[64];
 
-static int* next_sched_pair(int dev) { return g_sched[dev].pool + 2 * (g_sched[dev].seq.fetch_add(1) % kSchedSlots); }
+static int* next_sched_pair(int dev, cudaStream_t stream) {
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(stream, &cs) != cudaSuccess) { cudaGetLastError(); cs = cudaStreamCaptureStatusNone; }
+  DeviceSched& d = g_sched[dev];
+  if (cs == cudaStreamCaptureStatusActive) return d.pool + 2 * (kSchedSlots + d.seq_capture.fetch_add(1) % kSchedSlots);
+  return d.pool + 2 * (d.seq.fetch_add(1) % kSchedSlots);
+}
 
 int ensure_device(int* dev_out) {
   static std::mutex mu;
@@ -97,8 +109,8 @@ int ensure_device(int* dev_out) {
   SAP_CUDA_CHECK(cudaFuncSetAttribute(sap_bwd_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PairSmem::kTotal));
   SAP_CUDA_CHECK(cudaDeviceGetAttribute(&g_sched[dev].n_sms, cudaDevAttrMultiProcessorCount, dev));
   if (!g_sched[dev].pool) {
-    SAP_CUDA_CHECK(cudaMalloc(&g_sched[dev].pool, 2 * kSchedSlots * sizeof(int)));
-    SAP_CUDA_CHECK(cudaMemset(g_sched[dev].pool, 0, 2 * kSchedSlots * sizeof(int)));
+    SAP_CUDA_CHECK(cudaMalloc(&g_sched[dev].pool, 2 * 2 * kSchedSlots * sizeof(int)));   // eager pool | capture pool
+    SAP_CUDA_CHECK(cudaMemset(g_sched[dev].pool, 0, 2 * 2 * kSchedSlots * sizeof(int)));
   }
   ready.insert(dev);
   return SAP_OK;
@@ -190,7 +202,7 @@ static int launch_fwd(const DevProgram& prog, const void* q, const void* k, cons
     const unsigned grid = static_cast<unsigned>(n_work < g_sched[dev].n_sms ? n_work : g_sched[dev].n_sms);
     sap_fwd_pair_kernel<D, PARTIAL><<<grid, kFwdPairThreads, FwdPairSmem<D>::kTotal, stream>>>(
         mq, mk, mv, prog.tiles, prog.segs, cu, plan->n_docs, static_cast<__nv_bfloat16*>(out), out_f32, lse,
-        plan->n_tokens, Hq, Hkv, scale * kLog2e, prog.n_tiles, n_work, next_sched_pair(dev), 0);
+        plan->n_tokens, Hq, Hkv, scale * kLog2e, prog.n_tiles, n_work, next_sched_pair(dev, stream), 0);
   } else if (prog2 && prog2->n_tiles > 0 && ((g_fwd_form.load() == 0 && use_row_pairs(prog2->n_tiles, Hq)) || g_fwd_form.load() == 2)) {
     // odd Hq/Hkv (MHA): the same persistent kernel, its two units = the two 128-row halves of a 256-row tile of ONE q-head
     int dev = 0;
@@ -199,7 +211,7 @@ static int launch_fwd(const DevProgram& prog, const void* q, const void* k, cons
     const unsigned grid = static_cast<unsigned>(n_work < g_sched[dev].n_sms ? n_work : g_sched[dev].n_sms);
     sap_fwd_pair_kernel<D, PARTIAL><<<grid, kFwdPairThreads, FwdPairSmem<D>::kTotal, stream>>>(
         mq, mk, mv, prog2->tiles, prog2->segs, cu, plan->n_docs, static_cast<__nv_bfloat16*>(out), out_f32, lse,
-        plan->n_tokens, Hq, Hkv, scale * kLog2e, prog2->n_tiles, n_work, next_sched_pair(dev), 1);
+        plan->n_tokens, Hq, Hkv, scale * kLog2e, prog2->n_tiles, n_work, next_sched_pair(dev, stream), 1);
   } else {
     const unsigned grid = static_cast<unsigned>(prog.n_tiles) * Hq;
     sap_fwd_kernel<D, PARTIAL><<<grid, kFwdThreads, FwdSmem<D>::kTotal, stream>>>(
@@ -317,44 +329,99 @@ static int launch_bwd(const PlanDevice* pd, const void* dout, const void* q, con
 }
 
 // Range-restricted programs, built on first use of a range and kept with the plan (at most kMaxRangePrograms per
-// kind, least recently used evicted).  Uploads and evictions are ordered on the caller's stream: no synchronisation.
-static int get_range_program(sap_plan_t* plan, int kind, int32_t a, int32_t b, cudaStream_t stream, DevProgram* out) {
-  PlanDevice* pd = static_cast<PlanDevice*>(plan->dev_state);
-  std::lock_guard<std::mutex> lock(plan->mu);
-  auto& cache = pd->ranges[kind];
-  const auto key = std::make_pair(a, b);
-  RangeProgram* hit = nullptr;
-  for (auto it = cache.begin(); it != cache.end(); ++it)
-    if (it->key == key) { cache.splice(cache.begin(), cache, it); hit = &cache.front(); break; }
-  if (!hit) {
-    if (cache.size() >= kMaxRangePrograms) {
-      RangeProgram& old = cache.back();
-      if (old.dev.tiles) cudaFreeAsync(old.dev.tiles, stream);
-      if (old.dev.segs) cudaFreeAsync(old.dev.segs, stream);
-      if (old.ready) cudaEventDestroy(old.ready);
-      cache.pop_back();
-    }
-    cache.emplace_front();
-    RangeProgram& e = cache.front();
-    e.key = key;
-    const int32_t kv_rows = (kind == kRangeKvPair || kind == kRangeItemsKvPair) ? 2 * kTile : kTile;
-    switch (kind) {
-      case kRangeItemsQ: build_q_program(*plan, a, b, e.host); break;                                               // partial forward, every row
-      case kRangeItemsQDrop: build_q_program(*plan, a, b, e.host, true); break;                                     // ... touched Q tiles only
-      case kRangeQ: build_q_program(*plan, plan->chunk_offsets[a], plan->chunk_offsets[b], e.host, true); break;    // q-chunks
-      case kRangeQ2: build_q_program(*plan, plan->chunk_offsets[a], plan->chunk_offsets[b], e.host, true, 2 * kTile); break;   // ... in 256-row tiles
-      case kRangeKv: case kRangeKvPair: build_kv_program(*plan, e.host, a, b, kv_rows); break;                      // kv-chunks
-      default: build_kv_program(*plan, e.host, 0, -1, kv_rows, a, b, true); break;                                  // items, KV-stationary
-    }
-    e.stream = stream;
-    int rc = upload_program_async(e.host, e.dev, &e.ready, stream);
-    if (rc != SAP_OK) { cache.pop_front(); return rc; }
-    hit = &e;
-  }
-  if (hit->stream != stream) SAP_CUDA_CHECK(cudaStreamWaitEvent(stream, hit->ready, 0));
-  *out = hit->dev;
-  return SAP_OK;
+// kind; the least recently used one that no call and no CUDA graph holds is evicted).  Uploads and evictions are
+// ordered on streams: no synchronisation.
+static void destroy_range_program(RangeProgram& e) {   // immediate: the caller knows that nothing uses it any more
+  free_program(e.dev);
+  if (e.ready) cudaEventDestroy(e.ready);
+  for (auto& u : e.used) cudaEventDestroy(u.second);
+  e.used.clear();
 }
+
+// Frees an evicted program on `stream`, behind the last kernels that read it on every stream that used it.
+static void retire_range_program(RangeProgram& e, cudaStream_t stream) {
+  for (auto& u : e.used)
+    if (u.first != stream) cudaStreamWaitEvent(stream, u.second, 0);
+  if (e.stream != stream && e.ready) cudaStreamWaitEvent(stream, e.ready, 0);
+  if (e.dev.tiles) cudaFreeAsync(e.dev.tiles, stream);
+  if (e.dev.segs) cudaFreeAsync(e.dev.segs, stream);
+  e.dev = DevProgram();
+  destroy_range_program(e);   // cudaEventDestroy of a pending event is legal: the waits above are already enqueued
+}
+
+static bool stream_is_capturing(cudaStream_t stream) {
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(stream, &cs) != cudaSuccess) { cudaGetLastError(); return false; }
+  return cs == cudaStreamCaptureStatusActive;
+}
+
+// One call's hold on a cached range program: acquire() looks it up (or builds and uploads it) and pins it, the
+// destructor - after the call has enqueued its kernels - records the event eviction waits for and lets go.
+struct RangeUse {
+  sap_plan_t* plan = nullptr;
+  RangeProgram* entry = nullptr;
+  cudaStream_t stream = nullptr;
+  bool capturing = false;
+  DevProgram prog;
+
+  int acquire(sap_plan_t* p, int kind, int32_t a, int32_t b, cudaStream_t st) {
+    plan = p; stream = st;
+    capturing = stream_is_capturing(st);
+    PlanDevice* pd = static_cast<PlanDevice*>(plan->dev_state);
+    std::lock_guard<std::mutex> lock(plan->mu);
+    auto& cache = pd->ranges[kind];
+    const auto key = std::make_pair(a, b);
+    RangeProgram* hit = nullptr;
+    for (auto it = cache.begin(); it != cache.end(); ++it)
+      if (it->key == key) { cache.splice(cache.begin(), cache, it); hit = &cache.front(); break; }
+    if (!hit) {
+      // building a program allocates (cudaMallocAsync) and copies from pageable host memory: neither belongs in a graph
+      if (capturing) return SAP_ERR_UNSUPPORTED;
+      if (cache.size() >= kMaxRangePrograms)
+        for (auto it = cache.end(); it != cache.begin();) {   // least recently used first; held entries stay
+          --it;
+          if (it->pins == 0 && !it->held_by_graph) { retire_range_program(*it, stream); cache.erase(it); break; }
+        }
+      cache.emplace_front();
+      RangeProgram& e = cache.front();
+      e.key = key;
+      const int32_t kv_rows = (kind == kRangeKvPair || kind == kRangeItemsKvPair) ? 2 * kTile : kTile;
+      switch (kind) {
+        case kRangeItemsQ: build_q_program(*plan, a, b, e.host); break;                                               // partial forward, every row
+        case kRangeItemsQDrop: build_q_program(*plan, a, b, e.host, true); break;                                     // ... touched Q tiles only
+        case kRangeQ: build_q_program(*plan, plan->chunk_offsets[a], plan->chunk_offsets[b], e.host, true); break;    // q-chunks
+        case kRangeQ2: build_q_program(*plan, plan->chunk_offsets[a], plan->chunk_offsets[b], e.host, true, 2 * kTile); break;   // ... in 256-row tiles
+        case kRangeKv: case kRangeKvPair: build_kv_program(*plan, e.host, a, b, kv_rows); break;                      // kv-chunks
+        default: build_kv_program(*plan, e.host, 0, -1, kv_rows, a, b, true); break;                                  // items, KV-stationary
+      }
+      e.stream = stream;
+      int rc = upload_program_async(e.host, e.dev, &e.ready, stream);
+      if (rc != SAP_OK) { cache.pop_front(); return rc; }
+      hit = &e;
+    }
+    if (hit->stream != stream)   // a capturing stream may wait for an event from outside its graph only as an external one
+      SAP_CUDA_CHECK(cudaStreamWaitEvent(stream, hit->ready, capturing ? cudaEventWaitExternal : 0));
+    if (capturing) hit->held_by_graph = true;   // the graph will read it at every replay: never evicted
+    ++hit->pins;
+    entry = hit;
+    prog = hit->dev;
+    return SAP_OK;
+  }
+
+  ~RangeUse() {
+    if (!entry) return;
+    std::lock_guard<std::mutex> lock(plan->mu);
+    --entry->pins;
+    if (capturing) return;   // held_by_graph keeps it; an event recorded here would belong to the graph
+    cudaEvent_t ev = nullptr;
+    for (auto& u : entry->used) if (u.first == stream) ev = u.second;
+    if (!ev) {
+      if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); entry->held_by_graph = true; return; }
+      entry->used.emplace_back(stream, ev);
+    }
+    if (cudaEventRecord(ev, stream) != cudaSuccess) { cudaGetLastError(); entry->held_by_graph = true; }   // cannot order a free: keep it
+  }
+};
 
 static inline bool chunk_range_ok(const sap_plan_t* plan, int32_t a, int32_t b) { return a >= 0 && b >= a && b <= plan->n_chunks; }
 static inline bool item_range_ok(const sap_plan_t* plan, int32_t a, int32_t b) { return a >= 0 && b >= a && b <= (int32_t)plan->items.size(); }
@@ -463,7 +530,7 @@ void sap_plan_destroy(sap_plan_t* plan) {
     free_program(pd->kv2);
     free_program(pd->fwd2);
     for (auto& cache : pd->ranges)
-      for (auto& e : cache) { free_program(e.dev); if (e.ready) cudaEventDestroy(e.ready); }
+      for (auto& e : cache) destroy_range_program(e);
     if (switched) cudaSetDevice(cur);
     delete pd;
   }
@@ -502,8 +569,9 @@ int sap_attn_fwd_partial(const void* q, const void* k, const void* v, const int3
   if (!item_range_ok(plan, item_begin, item_end)) return SAP_ERR_INVALID_ARG;
   if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out_f32)) return SAP_ERR_UNSUPPORTED;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  DevProgram prog;
-  if ((rc = get_range_program(plan, kRangeItemsQ, item_begin, item_end, st, &prog)) != SAP_OK) return rc;
+  RangeUse use;
+  if ((rc = use.acquire(plan, kRangeItemsQ, item_begin, item_end, st)) != SAP_OK) return rc;
+  const DevProgram& prog = use.prog;
   if (head_dim == 128)
     return launch_fwd<128, true>(prog, q, k, v, cu_seqlens_dev, plan, nullptr, out_f32, lse, n_q_heads, n_kv_heads, softmax_scale, st);
   return launch_fwd<64, true>(prog, q, k, v, cu_seqlens_dev, plan, nullptr, out_f32, lse, n_q_heads, n_kv_heads, softmax_scale, st);
@@ -518,8 +586,9 @@ int sap_attn_fwd_items(const void* q, const void* k, const void* v, const int32_
   if (!item_range_ok(plan, item_begin, item_end)) return SAP_ERR_INVALID_ARG;
   if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out_f32)) return SAP_ERR_UNSUPPORTED;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  DevProgram prog;
-  if ((rc = get_range_program(plan, kRangeItemsQDrop, item_begin, item_end, st, &prog)) != SAP_OK) return rc;
+  RangeUse use;
+  if ((rc = use.acquire(plan, kRangeItemsQDrop, item_begin, item_end, st)) != SAP_OK) return rc;
+  const DevProgram& prog = use.prog;
   if (head_dim == 128)
     return launch_fwd<128, true>(prog, q, k, v, cu_seqlens_dev, plan, nullptr, out_f32, lse, n_q_heads, n_kv_heads, softmax_scale, st);
   return launch_fwd<64, true>(prog, q, k, v, cu_seqlens_dev, plan, nullptr, out_f32, lse, n_q_heads, n_kv_heads, softmax_scale, st);
@@ -581,11 +650,11 @@ int sap_attn_fwd_chunks(const void* q, const void* k, const void* v, const int32
   if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out)) return SAP_ERR_UNSUPPORTED;
   if (q_chunk_begin == q_chunk_end) return SAP_OK;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  DevProgram prog;
-  if ((rc = get_range_program(plan, kRangeQ, q_chunk_begin, q_chunk_end, st, &prog)) != SAP_OK) return rc;
-  DevProgram prog2;   // odd Hq/Hkv (MHA): the row-pair form needs the same rows in 256-row tiles
-  const bool odd = (n_q_heads / n_kv_heads) % 2 != 0;
-  if (odd && (rc = get_range_program(plan, kRangeQ2, q_chunk_begin, q_chunk_end, st, &prog2)) != SAP_OK) return rc;
+  RangeUse use, use2;
+  if ((rc = use.acquire(plan, kRangeQ, q_chunk_begin, q_chunk_end, st)) != SAP_OK) return rc;
+  const bool odd = (n_q_heads / n_kv_heads) % 2 != 0;   // odd Hq/Hkv (MHA): the row-pair form needs the same rows in 256-row tiles
+  if (odd && (rc = use2.acquire(plan, kRangeQ2, q_chunk_begin, q_chunk_end, st)) != SAP_OK) return rc;
+  const DevProgram &prog = use.prog, &prog2 = use2.prog;
   if (head_dim == 128)
     return launch_fwd<128, false>(prog, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st, odd ? &prog2 : nullptr);
   return launch_fwd<64, false>(prog, q, k, v, cu_seqlens_dev, plan, out, nullptr, lse, n_q_heads, n_kv_heads, softmax_scale, st, odd ? &prog2 : nullptr);
@@ -616,8 +685,9 @@ static int bwd_range(int kind1, int kind2, int32_t a, int32_t b, const void* dou
   int rc;
   if ((rc = bwd_ws(plan, Hq, Hkv, d, workspace, workspace_bytes, &dsum, &dq_acc)) != SAP_OK) return rc;
   if (a == b) return SAP_OK;
-  DevProgram prog;
-  if ((rc = get_range_program(plan, use_pair_kernel(d) ? kind2 : kind1, a, b, st, &prog)) != SAP_OK) return rc;
+  RangeUse use;
+  if ((rc = use.acquire(plan, use_pair_kernel(d) ? kind2 : kind1, a, b, st)) != SAP_OK) return rc;
+  const DevProgram& prog = use.prog;
   if (d == 128) return launch_bwd_main<128>(prog, prog, dout, q, k, v, lse, cu, plan, dk, dv, Hq, Hkv, scale, dsum, dq_acc, st);
   return launch_bwd_main<64>(prog, prog, dout, q, k, v, lse, cu, plan, dk, dv, Hq, Hkv, scale, dsum, dq_acc, st);
 }

@@ -70,6 +70,7 @@ __device__ __forceinline__ int fwd_tile_iters(const TileDesc& td, const SegDesc*
 
 // `sched` = {next, done}: two zero-initialised counters of this launch.  CTA b starts with item b and then takes item
 // gridDim.x + atomicAdd(next, 1); the last CTA to leave zeroes both again, so the pair can serve the next launch.
+// The host hands every launch a pair no other launch in flight holds (sap_api.cu: next_sched_pair).
 template <int D, bool PARTIAL>
 __global__ void __launch_bounds__(kFwdPairThreads, 1)
 sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
@@ -435,7 +436,15 @@ sap_fwd_pair_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
   if (warp == 1) tmem_dealloc(tmem, 512);
   if (threadIdx.x == 0) {   // the last CTA to leave re-arms the counters for the next launch
     __threadfence();
-    if (atomicAdd(sched + 1, 1) == static_cast<int>(gridDim.x) - 1) { sched[0] = 0; sched[1] = 0; __threadfence(); }
+    const int left = atomicAdd(sched + 1, 1);
+    // A pair serves ONE launch at a time (sap.h, sap_attn_fwd).  Every CTA draws from `next` until its draw misses, so a
+    // launch that had the pair to itself ends with done < gridDim.x and next == n_work; anything else means a second
+    // launch was drawing from the same pair and work items were skipped or done twice: stop loudly, not with wrong output.
+    if (left >= static_cast<int>(gridDim.x)) __trap();
+    if (left == static_cast<int>(gridDim.x) - 1) {
+      if (*reinterpret_cast<volatile int*>(sched) != n_work) __trap();
+      sched[0] = 0; sched[1] = 0; __threadfence();
+    }
   }
 }
 

@@ -6,6 +6,7 @@
 #include <atomic>
 #include <list>
 #include <utility>
+#include <vector>
 #include "sap_internal.h"
 
 namespace sap {
@@ -36,6 +37,12 @@ struct RangeProgram {
   DevProgram dev;
   cudaEvent_t ready = nullptr; // recorded behind the upload: other streams wait on it
   cudaStream_t stream = nullptr;
+  // Life time (sap_api.cu: RangeUse): a call pins the entry from lookup until its kernels are enqueued and then records
+  // an event behind them on its stream; eviction takes only unpinned entries and frees their memory behind all of
+  // those events.  An entry a CUDA graph has recorded a launch on stays until sap_plan_destroy.
+  int pins = 0;
+  bool held_by_graph = false;
+  std::vector<std::pair<cudaStream_t, cudaEvent_t>> used;   // last use per stream that ran kernels on this program
 };
 enum { kRangeItemsQ = 0, kRangeQ = 1, kRangeKv = 2, kRangeKvPair = 3, kRangeItemsKv = 4, kRangeItemsKvPair = 5, kRangeItemsQDrop = 6, kRangeQ2 = 7, kRangeKinds = 8 };
 

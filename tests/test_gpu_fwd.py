@@ -150,9 +150,10 @@ def test_fwd_rejects_bad_arguments():
 
 def test_fwd_persistent_scheduler_many_launches_two_streams():
     """The persistent forward takes its work items off {next, done} counter pairs that the last CTA of a launch re-arms
-    (sap_api.cu: kSchedSlots = 256 pairs per device, handed out round-robin).  600 launches - every pair reused - issued
-    alternately on two streams, so launches overlap: every one must reproduce the first result bit for bit (the
-    forward has no atomics on its outputs), with more work items than SMs and a ragged last tile."""
+    (sap_api.cu: kSchedSlots = 4096 pairs per device and pool, handed out round-robin).  4400 launches - every pair of the
+    eager pool reused - issued alternately on two streams, so launches overlap: every one must reproduce the first
+    result bit for bit (the forward has no atomics on its outputs), with more work items than SMs and a ragged last
+    tile.  A kernel that found its pair shared would trap and the final synchronize would raise."""
     w = custom_workload([3000, 1500, 2500 + 77, 1115], 4, 8, 2, 128, name="sched")
     q, k, v = (t.cuda() for t in make_qkv(w, device="cpu", with_dout=False))
     plan = sap.sap_plan(w.cu_seqlens, w.n_chunks)
@@ -162,7 +163,7 @@ def test_fwd_persistent_scheduler_many_launches_two_streams():
     streams = [torch.cuda.Stream(), torch.cuda.Stream()]
     outs = [[torch.empty_like(ref_out) for _ in range(3)] for _ in streams]
     lses = [[torch.empty_like(ref_lse) for _ in range(3)] for _ in streams]
-    for it in range(300):
+    for it in range(2200):
         for si, st in enumerate(streams):
             o, l = outs[si][it % 3], lses[si][it % 3]
             sap.sap_attn_fwd(q, k, v, cu, plan, out=o, lse=l, softmax_scale=w.softmax_scale, stream=st)
@@ -171,6 +172,42 @@ def test_fwd_persistent_scheduler_many_launches_two_streams():
         for j in range(3):
             assert torch.equal(outs[si][j], ref_out), f"stream {si} buffer {j}: out differs"
             assert torch.equal(lses[si][j], ref_lse), f"stream {si} buffer {j}: lse differs"
+
+
+def test_fwd_graph_replays_overlap_eager_launches():
+    """A forward recorded into a CUDA graph keeps its counter pair for the life of the graph, so it must come from a
+    pool that ordinary launches never draw from (sap.h, sap_attn_fwd): two graphs replayed on their own streams while a
+    third stream issues ordinary launches - more of them than the eager pool has pairs, so an eager launch would have
+    met a graph's pair had they shared a pool - must all reproduce the reference bit for bit."""
+    w = custom_workload([3000, 1500, 2500 + 77, 1115], 4, 8, 2, 128, name="sched_graph")
+    q, k, v = (t.cuda() for t in make_qkv(w, device="cpu", with_dout=False))
+    plan = sap.sap_plan(w.cu_seqlens, w.n_chunks)
+    cu = plan.cu_seqlens_dev("cuda")
+    ref_out, ref_lse = sap.sap_attn_fwd(q, k, v, cu, plan, softmax_scale=w.softmax_scale)
+    torch.cuda.synchronize()
+    graphs, g_out, g_lse, g_streams = [], [], [], []
+    for _ in range(2):
+        st = torch.cuda.Stream()
+        st.wait_stream(torch.cuda.current_stream())
+        o, l = torch.empty_like(ref_out), torch.empty_like(ref_lse)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(st):
+            with torch.cuda.graph(g, stream=st):
+                sap.sap_attn_fwd(q, k, v, cu, plan, out=o, lse=l, softmax_scale=w.softmax_scale)
+        graphs.append(g); g_out.append(o); g_lse.append(l); g_streams.append(st)
+    eager = torch.cuda.Stream()
+    e_out = [torch.empty_like(ref_out) for _ in range(3)]
+    e_lse = [torch.empty_like(ref_lse) for _ in range(3)]
+    torch.cuda.synchronize()
+    for it in range(4200):
+        if it % 4 == 0:
+            for g, st in zip(graphs, g_streams):
+                with torch.cuda.stream(st):
+                    g.replay()
+        sap.sap_attn_fwd(q, k, v, cu, plan, out=e_out[it % 3], lse=e_lse[it % 3], softmax_scale=w.softmax_scale, stream=eager)
+    torch.cuda.synchronize()
+    for o, l in zip(g_out + e_out, g_lse + e_lse):
+        assert torch.equal(o, ref_out) and torch.equal(l, ref_lse)
 
 
 @pytest.mark.parametrize("name", list(CASES))
@@ -189,3 +226,46 @@ def test_fwd_row_pair_form_matches_oracle(name):
     o_ref, l_ref = oracle.attn_fwd(to_np(q), to_np(k), to_np(v), w.cu_seqlens, w.softmax_scale)
     check_close(to_np(out), o_ref, f"{name}: out (row pairs)")
     check_lse(to_np(lse).T, l_ref, f"{name}: lse (row pairs)")
+
+
+def test_range_program_cache_eviction_two_streams_and_capture():
+    """Range-restricted programs are cached per plan, 64 per kind, and an evicted one is freed only behind the last kernel
+    that read it on EVERY stream (sap_api.cu: RangeUse).  136 one-item ranges - twice the cache - requested alternately on
+    two streams, so programs built on one stream are evicted by calls on the other while their kernels are still queued:
+    every partial must equal the one computed on a quiet device.  Then: the first use of a range inside stream capture
+    is refused (building a program allocates and copies from pageable memory), a range seen before can be captured."""
+    w = custom_workload([16 * 128], 16, 2, 2, 64, name="ranges")
+    q, k, v = (t.cuda() for t in make_qkv(w, device="cpu", with_dout=False))
+    plan = sap.sap_plan(w.cu_seqlens, w.n_chunks)
+    cu = plan.cu_seqlens_dev("cuda")
+    n = plan.n_items
+    assert n == 136
+    ref = []
+    for it in range(n):
+        ref.append(sap.sap_attn_fwd_partial(q, k, v, cu, plan, it, it + 1, softmax_scale=w.softmax_scale))
+        torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    got = []
+    for rep in range(2):
+        for it in range(n):
+            st = streams[(it + rep) % 2]
+            with torch.cuda.stream(st):     # the result tensors are allocated on the stream that fills them
+                got.append((it, sap.sap_attn_fwd_partial(q, k, v, cu, plan, it, it + 1, softmax_scale=w.softmax_scale, stream=st)))
+    torch.cuda.synchronize()
+    for it, (o, l) in got:
+        assert torch.equal(o, ref[it][0]) and torch.equal(l, ref[it][1]), f"item {it}"
+    # capture: item 0 was evicted long ago (miss), item n - 1 is in the cache (hit)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    o_g, l_g = torch.empty_like(ref[0][0]), torch.empty_like(ref[0][1])
+    graph = torch.cuda.CUDAGraph()
+    L = sap.api._lib.lib()
+    args = lambda it: (q.data_ptr(), k.data_ptr(), v.data_ptr(), cu.data_ptr(), plan.handle, w.n_tokens, it, it + 1, o_g.data_ptr(),
+                       l_g.data_ptr(), 2, 2, 64, float(w.softmax_scale), side.cuda_stream)
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            assert L.sap_attn_fwd_partial(*args(0)) == 4           # SAP_ERR_UNSUPPORTED, and the capture is still intact
+            assert L.sap_attn_fwd_partial(*args(n - 1)) == 0
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(o_g, ref[n - 1][0]) and torch.equal(l_g, ref[n - 1][1])
