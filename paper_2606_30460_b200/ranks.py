@@ -153,13 +153,23 @@ class RankGroup:
 # ---------------------------------------------------------------------------------------------------------------------
 # One process per GPU (the launch model of torch.distributed): the same phases, the barriers are group barriers of the
 # process group, and the stitched ranges are assembled from chunks the processes export to one another.
+_MAX_FDS_PER_MESSAGE = 253      # Linux SCM_MAX_FD: one sendmsg carries at most this many descriptors
+
+
 def exchange_fds(rank: int, world: int, my_fds: Dict[int, int], group=None, tag: str = "sap") -> Dict[int, Dict[int, int]]:
     """Every rank hands the file descriptors `my_fds` (key -> fd, e.g. the exported chunks it owns) to every other
     rank: descriptors only travel between processes of one host over a Unix socket (SCM_RIGHTS).  Returns
     {sender rank: {key: fd valid in THIS process}}; the receiver closes them once imported.  Needs an initialised
-    torch.distributed group (any backend: used for two barriers only)."""
+    torch.distributed group (any backend: used for one broadcast and two barriers).
+
+    The sockets live in a directory rank 0 creates for this exchange with mode 0700 (mkdtemp) and names to the others
+    through the process group, so no other user can connect.  A message is accepted only from a process of this user
+    (SO_PEERCRED), from a rank of the group that has not sent yet, and only whole: key count, payload length and the
+    number of descriptors must agree and the ancillary data must not be truncated.  Anything else raises; descriptors
+    received up to then are closed."""
     import array
     import os
+    import shutil
     import socket
     import struct
     import tempfile
@@ -167,39 +177,73 @@ def exchange_fds(rank: int, world: int, my_fds: Dict[int, int], group=None, tag:
 
     if world == 1:
         return {}
-    base = os.path.join(tempfile.gettempdir(), f"{tag}_fd_{os.environ.get('MASTER_PORT', '0')}_")
-    path = base + str(rank)
-    if os.path.exists(path):
-        os.unlink(path)
+    if len(my_fds) > _MAX_FDS_PER_MESSAGE:
+        raise ValueError(f"at most {_MAX_FDS_PER_MESSAGE} descriptors per exchange, got {len(my_fds)}")
+    box = [tempfile.mkdtemp(prefix=f"{tag}_fd_") if rank == 0 else None]
+    dist.broadcast_object_list(box, src=0 if group is None else dist.get_global_rank(group, 0), group=group)
+    root = box[0]
+    path = os.path.join(root, str(rank))
     srv = socket.socket(socket.AF_UNIX, socket.SOCK_STREAM)
-    srv.bind(path)
-    srv.listen(world)
-    dist.barrier(group=group)                      # every rank listens
-    keys = sorted(my_fds)
-    for peer in range(world):                      # send to everybody (small messages: the connects do not block)
-        if peer == rank:
-            continue
-        c = socket.socket(socket.AF_UNIX, socket.SOCK_STREAM)
-        c.connect(base + str(peer))
-        payload = struct.pack(f"<ii{len(keys)}i", rank, len(keys), *keys)
-        fds = array.array("i", [my_fds[k] for k in keys])
-        c.sendmsg([payload], [(socket.SOL_SOCKET, socket.SCM_RIGHTS, fds)] if keys else [])
-        c.close()
     got: Dict[int, Dict[int, int]] = {}
-    for _ in range(world - 1):
-        conn, _addr = srv.accept()
-        msg, anc, _flags, _a = conn.recvmsg(4096, socket.CMSG_SPACE(4 * 256))
-        sender, n = struct.unpack_from("<ii", msg)
-        ks = struct.unpack_from(f"<{n}i", msg, 8)
-        fds = array.array("i")
-        for level, typ, data in anc:
-            if level == socket.SOL_SOCKET and typ == socket.SCM_RIGHTS:
-                fds.frombytes(data[: len(data) - (len(data) % fds.itemsize)])
-        got[sender] = dict(zip(ks, list(fds)))
-        conn.close()
-    dist.barrier(group=group)                      # every rank has received
-    srv.close()
-    os.unlink(path)
+
+    def fail(why):
+        for fds in got.values():
+            for fd in fds.values():
+                os.close(fd)
+        raise RuntimeError(f"exchange_fds (rank {rank}): {why}")
+
+    try:
+        srv.bind(path)
+        srv.listen(world)
+        dist.barrier(group=group)                      # every rank listens
+        keys = sorted(my_fds)
+        for peer in range(world):                      # send to everybody (small messages: the connects do not block)
+            if peer == rank:
+                continue
+            c = socket.socket(socket.AF_UNIX, socket.SOCK_STREAM)
+            c.connect(os.path.join(root, str(peer)))
+            payload = struct.pack(f"<ii{len(keys)}i", rank, len(keys), *keys)
+            fds = array.array("i", [my_fds[k] for k in keys])
+            c.sendmsg([payload], [(socket.SOL_SOCKET, socket.SCM_RIGHTS, fds)] if keys else [])
+            c.close()
+        for _ in range(world - 1):
+            conn, _addr = srv.accept()
+            try:
+                _pid, uid, _gid = struct.unpack("3i", conn.getsockopt(socket.SOL_SOCKET, socket.SO_PEERCRED, struct.calcsize("3i")))
+                msg, anc, flags, _a = conn.recvmsg(8 + 4 * _MAX_FDS_PER_MESSAGE, socket.CMSG_SPACE(4 * _MAX_FDS_PER_MESSAGE))
+            finally:
+                conn.close()
+            fds = array.array("i")
+            for level, typ, data in anc:
+                if level == socket.SOL_SOCKET and typ == socket.SCM_RIGHTS:
+                    fds.frombytes(data[: len(data) - (len(data) % fds.itemsize)])
+            fds = list(fds)
+            sender, n = struct.unpack_from("<ii", msg) if len(msg) >= 8 else (-1, -1)
+            ok = (uid == os.getuid() and not (flags & (socket.MSG_CTRUNC | socket.MSG_TRUNC)) and 0 <= sender < world and
+                  sender != rank and sender not in got and 0 <= n <= _MAX_FDS_PER_MESSAGE and len(msg) == 8 + 4 * n and len(fds) == n)
+            if not ok:
+                for fd in fds:
+                    os.close(fd)
+                fail(f"malformed or foreign message (uid {uid}, sender {sender}, {n} keys, {len(msg)} bytes, {len(fds)} descriptors, "
+                     f"flags {flags:#x})")
+            ks = struct.unpack_from(f"<{n}i", msg, 8)
+            if len(set(ks)) != n:
+                for fd in fds:
+                    os.close(fd)
+                fail(f"rank {sender} sent duplicate keys")
+            got[sender] = dict(zip(ks, fds))
+        dist.barrier(group=group)                      # every rank has received
+    except BaseException:
+        if rank == 0:                                  # nobody will reach the closing barrier: do not leave the directory behind
+            shutil.rmtree(root, ignore_errors=True)
+        raise
+    finally:
+        srv.close()
+        if os.path.exists(path):
+            os.unlink(path)
+    dist.barrier(group=group)                          # every socket is gone: rank 0 removes the directory
+    if rank == 0:
+        shutil.rmtree(root, ignore_errors=True)
     return got
 
 
@@ -282,12 +326,24 @@ class ProcessRank:
         mine = {c: s.export_fd(c) for c in range(n_chunks) if own[c]}
         self._n_ranges += 1
         theirs = exchange_fds(self.rank, self.world, mine, self.group, tag=f"sap{self._n_ranges}")
-        for _sender, fds in theirs.items():
-            for c, fd in fds.items():
-                s.import_fd(c, fd)
+        seen = set(mine)
+        try:
+            for sender, fds in theirs.items():
+                for c, fd in fds.items():
+                    if not 0 <= c < n_chunks or c in seen:
+                        raise RuntimeError(f"rank {sender} sent chunk {c}, which is out of range or already mapped")
+                    s.import_fd(c, fd)
+                    seen.add(c)
+        finally:
+            for fds in theirs.values():
+                for fd in fds.values():
+                    os.close(fd)
+            for fd in mine.values():
                 os.close(fd)
-        for fd in mine.values():
-            os.close(fd)
+        # a chunk nobody exported would stay an unmapped hole in the range: the kernels would fault on it much later
+        missing = [c for c in range(n_chunks) if c not in seen]
+        if missing:
+            raise RuntimeError(f"rank {self.rank}: no process exported chunks {missing} of a {n_chunks}-chunk range")
         return s
 
     def tensor(self, tail_shape: Sequence[int], dtype):

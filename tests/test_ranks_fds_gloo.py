@@ -52,6 +52,55 @@ def test_three_ranks_exchange_descriptors():
         assert res[rank] == {sk: v for sk, v in want.items() if sk[0] != rank}, (rank, res[rank])
 
 
+def _bad_peer_worker(rank, world, port, q):
+    """rank 1 speaks the protocol by hand and announces two keys while attaching one descriptor; rank 0 must refuse"""
+    import array
+    import struct
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        if rank == 0:
+            from paper_2606_30460_b200.ranks import exchange_fds
+            try:
+                exchange_fds(0, 2, {})
+                q.put("accepted")
+            except RuntimeError as e:
+                q.put(str(e))
+        else:
+            box = [None]
+            dist.broadcast_object_list(box, src=0)
+            assert oct(os.stat(box[0]).st_mode & 0o777) == "0o700"      # private to this user
+            srv = socket.socket(socket.AF_UNIX, socket.SOCK_STREAM)     # rank 0 sends its (empty) message here
+            srv.bind(os.path.join(box[0], "1"))
+            srv.listen(2)
+            dist.barrier()
+            with tempfile.TemporaryFile() as f:
+                c = socket.socket(socket.AF_UNIX, socket.SOCK_STREAM)
+                c.connect(os.path.join(box[0], "0"))
+                c.sendmsg([struct.pack("<iiii", 1, 2, 7, 8)], [(socket.SOL_SOCKET, socket.SCM_RIGHTS, array.array("i", [f.fileno()]))])
+                c.close()
+    finally:
+        dist.destroy_process_group()
+
+
+def test_incomplete_message_is_refused():
+    from paper_2606_30460_b200.ranks import exchange_fds
+    import pytest
+    with pytest.raises(ValueError):          # more descriptors than one SCM_RIGHTS message carries: refused before anything is sent
+        exchange_fds(0, 2, {i: 0 for i in range(254)})
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_bad_peer_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    msg = q.get(timeout=120)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    assert "malformed or foreign message" in msg and "2 keys" in msg and "1 descriptors" in msg, msg
+
+
 def test_launch_chunks_cover_every_chunk_once_and_balance_the_causal_load():
     """ranks.launch_chunks: a partition of the chunks; with one document over the whole sequence the work of q-chunk c
     is c + 1 blocks, and zig-zag brings every rank to the same total where contiguous ownership does not."""
