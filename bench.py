@@ -190,9 +190,8 @@ def d64_context(dev, steps: int = 3):
     forward keeps the MUFU (16 exp / clk / SM) over 80 % busy and cannot reach the d = 128 rate."""
     import torch
     import paper_2606_30460_b200 as sap
-    from paper_2606_30460_b200.workloads import custom_workload, make_qkv, make_workload
-    w0 = make_workload(3)
-    w = custom_workload(w0.doc_lens, w0.n_chunks, 64, 16, 64, name="configs[2] packing, 64/16 heads, d=64")
+    from paper_2606_30460_b200.workloads import make_d64_workload, make_qkv
+    w = make_d64_workload()     # parity at this size: tests/test_gpu_configs.py::test_d64_context_workload_sampled_against_oracle
     q, k, v, do = make_qkv(w, device=dev)
     plan = sap.sap_plan(w.cu_seqlens, w.n_chunks); plan.upload()
     cu = plan.cu_seqlens_dev(dev)

@@ -161,6 +161,13 @@ def make_table2_workload(seq_len: int, seed: int = 0) -> Workload:
                     tuple(docs), seed)
 
 
+def make_d64_workload() -> Workload:
+    """SURVEY 8(f) NEXT-4, head_dim 64: configs[2]'s packing with 64 q-heads on 16 kv-heads of 64 (the same bytes per
+    token as configs[2]).  What bench.py's `d64_context` times and tests/test_gpu_configs.py checks."""
+    w0 = make_workload(3)
+    return custom_workload(w0.doc_lens, w0.n_chunks, 64, 16, 64, seed=w0.seed, name="configs[2] packing, 64/16 heads, d=64")
+
+
 def custom_workload(doc_lens: Sequence[int], n_chunks: int, n_q_heads: int, n_kv_heads: int,
                     head_dim: int, seed: int = 0, name: str = "custom") -> Workload:
     return Workload(name, int(sum(doc_lens)), n_chunks, n_q_heads, n_kv_heads, head_dim,

@@ -21,7 +21,7 @@ import torch
 
 import paper_2606_30460_b200 as sap
 from oracle import oracle
-from paper_2606_30460_b200.workloads import make_qkv, make_workload
+from paper_2606_30460_b200.workloads import make_d64_workload, make_qkv, make_workload
 from parity import check_close, check_lse, to_np, row_scale, col_scale
 
 pytestmark = pytest.mark.gpu
@@ -60,11 +60,23 @@ def sample_cols(w, rng):
 @pytest.mark.parametrize("cfg", [2, 3, 4, 5])
 def test_full_size_config_sampled_against_oracle(cfg):
     kv_sel, n_random, n_live = PLAN[cfg]
-    w = make_workload(cfg)
+    check_full_size(make_workload(cfg), cfg, kv_sel, n_random, n_live, 100 + cfg)
+
+
+def test_d64_context_workload_sampled_against_oracle():
+    """head_dim 64 at the size bench.py reports it (`d64_context`: configs[2]'s 128K packing, 64 q-heads on 16 kv-heads):
+    the persistent pair forward at d = 64 and sap_bwd_fused_kernel<64> over documents of up to ~1000 streamed tiles per
+    row, where the small d = 64 cases stop at 9.  Same sampling as the configs above."""
+    w = make_d64_workload()
+    assert (w.n_tokens, w.n_q_heads, w.n_kv_heads, w.head_dim) == (131072, 64, 16, 64)
+    check_full_size(w, "d64", (3, 11), 384, 384, 164)
+
+
+def check_full_size(w, cfg, kv_sel, n_random, n_live, seed):
     N, Hq, Hkv, d = w.n_tokens, w.n_q_heads, w.n_kv_heads, w.head_dim
     g = Hq // Hkv
     q_sel = [hk * g + i for hk in kv_sel for i in range(g)]
-    rng = np.random.default_rng(100 + cfg)
+    rng = np.random.default_rng(seed)
     q, k, v, do = make_qkv(w, device="cuda")
     plan = sap.sap_plan(w.cu_seqlens, w.n_chunks)
     ref_plan = oracle.plan(w.cu_seqlens, w.n_chunks)
