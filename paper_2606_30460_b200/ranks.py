@@ -289,6 +289,72 @@ def assign_by_work(work: Sequence[int], world: int) -> List[List[int]]:
     return [sorted(x) for x in out]
 
 
+def link_bytes(cu_seqlens: Sequence[int], n_chunks: int, world: int, design: str, n_q_heads: int, n_kv_heads: int,
+               head_dim: int) -> List[Dict[str, int]]:
+    """Bytes each rank moves over NVLink in one forward + backward, counted from the tile programs the kernels walk
+    (sap_debug_tile_program), with contiguous ownership (rank r owns and launches chunks [r P/W, (r+1) P/W)).  Host only.
+
+    design "stitched" (RankGroup / ProcessRank): tensors are read where they live.  A rank's kernel loads every
+        streamed tile it needs through TMA; a tile in a peer's memory is cached in the OWNER's L2, not the reader's, so
+        each load of it crosses the link - the reuse that keeps the one-GPU DRAM traffic low turns into link traffic.
+          forward  : per (Q tile, streamed 128-key tile, work item): K + V tile = 2 * 128 * d * 2 B; work items per tile =
+                     Hq / 2 when Hq / Hkv is even (two q-heads of a group share the stream), Hq otherwise
+          backward : per (K/V tile, streamed 128-row tile, q-head): Q + dO tile = 2 * 128 * d * 2 B plus LSE and D
+                     (2 * 128 * 4 B) read, and 128 * d * 4 B of fp32 dQ contributions sent with red.global to the
+                     owner of the rows (ranks.workspace_units keeps the accumulator rows with the chunk's owner)
+    design "staged" (the paper's own exchange; executor.py / ring.py): every remote shard a
+        rank needs travels ONCE into local staging and the kernels run on local memory.
+          forward  : K_j, V_j rows [kv_begin, kv_end) of every remote chunk j some owned q-chunk has an item against
+          backward : K/V-stationary at the owner of j: Q_i, dO_i (+ LSE, D) rows [q_begin, q_end) of every remote chunk
+                     i, once, and one fp32 dQ partial of those rows sent back (Table 1 copy-dq, :95-98)
+    Returns per rank {"fwd_read", "bwd_read", "bwd_red"} in bytes ("bwd_red": red.global traffic / dQ partials SENT).
+    Tile rows past the end of a document are counted as loaded (the kernels load whole boxes)."""
+    import numpy as np
+    if design not in ("stitched", "staged"):
+        raise ValueError("design is 'stitched' or 'staged'")
+    if n_chunks % world != 0:
+        raise ValueError("n_chunks must be a multiple of the number of ranks")
+    plan = api.sap_plan(cu_seqlens, n_chunks)
+    N, per = plan.n_tokens, n_chunks // world
+    n = N // n_chunks
+    owner = lambda t: min(t // n, n_chunks - 1) // per          # rank that owns token t
+    Hq, Hkv, d = int(n_q_heads), int(n_kv_heads), int(head_dim)
+    out = [{"fwd_read": 0, "bwd_read": 0, "bwd_red": 0} for _ in range(world)]
+    if design == "staged":
+        items = plan.items
+        for r in range(world):
+            mine = range(r * per, (r + 1) * per)
+            kv_span: Dict[int, List[int]] = {}      # remote kv-chunk j -> [lo, hi) over the items of my q-chunks
+            q_span: Dict[int, List[int]] = {}       # remote q-chunk i -> [lo, hi) over the items of my kv-chunks
+            for i, j, _dl, _dh, _kind, _step, qb, qe, kb, ke in items.tolist():
+                if i in mine and j not in mine:
+                    sp = kv_span.setdefault(j, [kb, ke]); sp[0] = min(sp[0], kb); sp[1] = max(sp[1], ke)
+                if j in mine and i not in mine:
+                    sp = q_span.setdefault(i, [qb, qe]); sp[0] = min(sp[0], qb); sp[1] = max(sp[1], qe)
+            out[r]["fwd_read"] = sum(hi - lo for lo, hi in kv_span.values()) * Hkv * d * 2 * 2
+            rows = sum(hi - lo for lo, hi in q_span.values())
+            out[r]["bwd_read"] = rows * Hq * (d * 2 * 2 + 2 * 4)
+            out[r]["bwd_red"] = rows * Hq * d * 4
+        return out
+    share = 2 if (Hq // Hkv) % 2 == 0 else 1
+    kv_kind = 7 if d == 128 else 6              # 256-key pair-tiles at head_dim 128, 128-key tiles otherwise
+    for r in range(world):
+        tiles, segs = plan.tile_program(5, r * per, (r + 1) * per)
+        loads = 0
+        for _row0, _rows, sb, se in tiles.tolist():
+            for tb, te, *_ in segs[sb:se].tolist():
+                loads += sum(1 for t in range(tb, te, 128) if owner(t) != r)
+        out[r]["fwd_read"] = loads * (Hq // share) * 2 * 128 * d * 2
+        tiles, segs = plan.tile_program(kv_kind, r * per, (r + 1) * per)
+        loads = 0
+        for _row0, _rows, sb, se in tiles.tolist():
+            for tb, te, *_ in segs[sb:se].tolist():
+                loads += sum(1 for t in range(tb, te, 128) if owner(t) != r)
+        out[r]["bwd_read"] = loads * Hq * (2 * 128 * d * 2 + 2 * 128 * 4)
+        out[r]["bwd_red"] = loads * Hq * 128 * d * 4
+    return out
+
+
 class ProcessRank:
     """This process = SAP rank `rank` of `world` on its own CUDA device.  The sequence has n_chunks chunks (a multiple of
     world; default one per rank); the rank OWNS the memory of a contiguous block of them and LAUNCHES the
