@@ -174,6 +174,11 @@ def shard_view_ok(n: int, head_dim: int = 0, backward: bool = False) -> bool:
     return n > 0 and n % tile == 0
 
 
+def _ws_bytes(plan, Hq, Hkv, d):
+    from . import api
+    return api.sap_workspace_bytes(plan, Hq, Hkv, d, api.SAP_PASS_BWD)
+
+
 def _max_inflight(code_lists, tensor_kinds):
     """largest number of same-kind RECVs one rank has in one stage: the 'fixed multiple' of a shard the staging area
     needs (PAPER.md:140)"""
@@ -229,12 +234,29 @@ class LocalExecutor:
         self.comp_q = e(P, n, Hq, d); self.comp_kv = e(P, 2, n, Hkv, d)
         self.comp_do = e(P, n, Hq, d); self.comp_dol = e(P, 2, Hq, n, dtype=f32)
         self.part_o = e(n, Hq, d, dtype=f32); self.part_l = e(Hq, self.N, dtype=f32)              # one partial result
+        self.part_lc = e(Hq, n, dtype=f32)                                                         # its LSE rows, shard-sized
         self.scratch_dkv = e(2, n, Hkv, d)
+        # what a rank computed for another rank waits here until the next stage's SEND: a rank runs one item per stage and
+        # its result leaves one stage later, so one slot per rank and kind is enough
+        self.out_o = e(P, n, Hq, d, dtype=f32); self.out_ol = e(P, Hq, n, dtype=f32)
+        self.out_dq = e(P, n, Hq, d, dtype=f32); self.out_dkv = e(P, 2, n, Hkv, d)
+        # running results of all P ranks, and the backward workspaces.  The C ABI lays a workspace out as D [Hq, N] followed by
+        # the accumulator [N, Hq, d] from ONE base pointer and addresses both by global token, so even the helper's scratch
+        # workspace has to be full length (a rank proper would need its own rows plus one shard); they are allocated once.
+        self.acc_o = e(P, n, Hq, d, dtype=f32); self.acc_l = e(P, Hq, n, dtype=f32)
+        need = _ws_bytes(plan, Hq, Hkv, d)
+        self.ws_own = torch.empty(need, dtype=torch.uint8, device=device)     # owners' D and dQ accumulator rows
+        self.ws_help = torch.empty(need, dtype=torch.uint8, device=device)    # scratch of the rank that helps another
+        self.dkv_tot = e(2, self.N, Hkv, d, dtype=f32)
+        self.mem_marks = []       # torch.cuda.memory_allocated() at the start of every stage of the last replay (tests)
 
     # ------------------------------------------------------------------------------------------------ helpers
     def _walk(self, code_lists, on_transfer, on_compute, on_copy):
+        import torch
         stages = sorted(set(int(c[0]) for codes in code_lists for c in codes))
+        self.mem_marks = []
         for st in stages:
+            self.mem_marks.append(torch.cuda.memory_allocated(self.dev))
             per_rank = [[tuple(int(v) for v in c) for c in codes if int(c[0]) == st] for codes in code_lists]
             sends = {(tensor, r, peer, item) for r, mine in enumerate(per_rank) for _, op, tensor, peer, item in mine if op == SAP_OP_SEND}
             recvs = [(tensor, peer, r, item) for r, mine in enumerate(per_rank) for _, op, tensor, peer, item in mine if op == SAP_OP_RECV]
@@ -252,6 +274,7 @@ class LocalExecutor:
                 for _, op, tensor, peer, item in mine:
                     if op == SAP_OP_COPY:
                         on_copy(r, tensor, peer, item, slot_of[(tensor, peer, r, item)])
+        self.mem_marks.append(torch.cuda.memory_allocated(self.dev))
 
     # ------------------------------------------------------------------------------------------------ forward
     def forward(self, q, k, v, cu_seqlens_dev):
@@ -262,8 +285,7 @@ class LocalExecutor:
         n, N, P, Hq = self.n, self.N, self.P, self.Hq
         own_q = lambda r: q[r * n:(r + 1) * n]
         own_kv = lambda r: (k[r * n:(r + 1) * n], v[r * n:(r + 1) * n])
-        acc_o = torch.zeros((P, n, Hq, self.d), dtype=torch.float32, device=self.dev)
-        acc_l = torch.full((P, Hq, n), float("-inf"), dtype=torch.float32, device=self.dev)
+        acc_o, acc_l = self.acc_o.zero_(), self.acc_l.fill_(float("-inf"))
         have_q, have_kv, results = {}, {}, {}      # (rank, item) -> operand in the compute buffer; helper partials
 
         def merge(r, item, o, l):
@@ -298,11 +320,12 @@ class LocalExecutor:
             qg, kg, vg = ShardView(qs.contiguous(), i * n, N), ShardView(ks.contiguous(), j * n, N), ShardView(vs.contiguous(), j * n, N)
             api.sap_attn_fwd_items(qg, kg, vg, cu_seqlens_dev, self.plan, item, item + 1, ShardView(self.part_o, i * n, N),
                                           self.part_l, Hq, self.Hkv, self.d, softmax_scale=self.scale)
-            o, l = self.part_o, self.part_l[:, i * n:(i + 1) * n].contiguous()
+            o, l = self.part_o, self.part_lc.copy_(self.part_l[:, i * n:(i + 1) * n])
             if i == r:
                 merge(r, item, o, l)
-            else:
-                results[(r, item)] = (o.clone(), l)          # a helper's partial: travels back one stage later
+            else:                                            # a helper's partial: travels back one stage later
+                assert not any(key[0] == r for key in results), f"rank {r}: its previous partial result has not been sent yet"
+                results[(r, item)] = (self.out_o[r].copy_(o), self.out_ol[r].copy_(l))
 
         def on_copy(r, tensor, peer, item, slot):
             if tensor == SAP_T_Q:
@@ -324,15 +347,13 @@ class LocalExecutor:
         import torch
         from . import api
         n, N, P, Hq, Hkv, d = self.n, self.N, self.P, self.Hq, self.Hkv, self.d
-        need = api.sap_workspace_bytes(self.plan, Hq, Hkv, d, 1)
-        ws_own = torch.empty(need, dtype=torch.uint8, device=self.dev)    # owners' D and dQ accumulator rows
-        ws_help = torch.empty(need, dtype=torch.uint8, device=self.dev)   # scratch of the rank that helps another
+        ws_own, ws_help = self.ws_own, self.ws_help
         acc_off = ((N * Hq * 4 + 255) // 256) * 256
         dsum = lambda ws: ws[:N * Hq * 4].view(torch.float32).view(Hq, N)
         dqacc = lambda ws: ws[acc_off:acc_off + N * Hq * d * 4].view(torch.float32).view(N, Hq, d)
         for r in range(P):   # every rank: D of its rows, zero its accumulator rows (sap_attn_bwd_begin)
             api.sap_attn_bwd_begin(dout, out, self.plan, r, r + 1, Hkv, ws_own)
-        dkv_tot = torch.zeros((2, N, Hkv, d), dtype=torch.float32, device=self.dev)
+        dkv_tot = self.dkv_tot.zero_()
         have, results = {}, {}
         own = lambda t, r: t[r * n:(r + 1) * n]
 
@@ -374,10 +395,12 @@ class LocalExecutor:
                 api.sap_axpy(dkv_tot[0, j * n + kb:j * n + ke], self.scratch_dkv[0, kb:ke], 1.0)
                 api.sap_axpy(dkv_tot[1, j * n + kb:j * n + ke], self.scratch_dkv[1, kb:ke], 1.0)
             else:
-                c = torch.zeros_like(self.scratch_dkv); c[:, kb:ke] = self.scratch_dkv[:, kb:ke]
+                assert not any(key[0] == r for key in results), f"rank {r}: its previous contribution has not been sent yet"
+                c = self.out_dkv[r].zero_(); c[:, kb:ke].copy_(self.scratch_dkv[:, kb:ke])
                 results[(r, SAP_T_DKV, item)] = c
             if i != r:
-                results[(r, SAP_T_DQ, item)] = dqacc(ws)[i * n:(i + 1) * n].clone()
+                assert not any(key[0] == r for key in results), f"rank {r}: its previous contribution has not been sent yet"
+                results[(r, SAP_T_DQ, item)] = self.out_dq[r].copy_(dqacc(ws)[i * n:(i + 1) * n])
 
         def on_copy(r, tensor, peer, item, slot):
             if tensor == SAP_T_Q:

@@ -53,6 +53,34 @@ def test_replay_all_ranks_small(case, policy):
 
 
 @pytest.mark.parametrize("policy", [sap.SAP_SCHED_RING, sap.SAP_SCHED_BALANCED])
+def test_replay_runs_in_buffers_allocated_once(policy):
+    """"fixed global buffer ... no memory jitter".  Everything a replay needs - staging slots, compute
+    buffers, the slots results wait in for their SEND, running results, workspaces - is allocated by LocalExecutor's
+    constructor: device memory in use is the same at the start of every stage and after the last one, and over a whole
+    forward / backward the peak exceeds the starting level by exactly the tensors the call returns."""
+    w = custom_workload([2048], 8, 2, 1, 128, name="fixed_buffers")      # one document over 8 ranks: helpers in both passes
+    q, k, v, do = make_qkv(w, device="cuda")
+    plan = sap.sap_plan(w.cu_seqlens, w.n_chunks)
+    cu = plan.cu_seqlens_dev("cuda")
+    slots, _ = plan.schedule(policy)
+    ex = executor.LocalExecutor(plan, slots, w.n_q_heads, w.n_kv_heads, w.head_dim, q.device, softmax_scale=w.softmax_scale)
+    out, lse = ex.forward(q, k, v, cu)                # first use: range programs are built and uploaded by the library
+    dq, dk, dv = ex.backward(do, q, k, v, out, lse, cu)
+    del dq, dk, dv
+    torch.cuda.synchronize()
+    nbytes = lambda *ts: sum(t.numel() * t.element_size() for t in ts)
+    for call, returned in ((lambda: ex.forward(q, k, v, cu), nbytes(out, lse)),
+                           (lambda: ex.backward(do, q, k, v, out, lse, cu), nbytes(q, k, v))):
+        base = torch.cuda.memory_allocated()
+        torch.cuda.reset_peak_memory_stats()
+        res = call()
+        torch.cuda.synchronize()
+        assert len(ex.mem_marks) >= 3 and set(ex.mem_marks) == {base}, ex.mem_marks
+        assert torch.cuda.max_memory_allocated() - base <= returned + 4096 * len(res), (torch.cuda.max_memory_allocated() - base, returned)
+        del res
+
+
+@pytest.mark.parametrize("policy", [sap.SAP_SCHED_RING, sap.SAP_SCHED_BALANCED])
 def test_replay_all_ranks_cfg2_equals_single_launch(policy):
     # BASELINE.json configs[1] at full size: the replay must reproduce the one-launch path (itself checked against the
     # oracle in test_gpu_configs.py) - out / dK / dV up to the rounding of the extra bf16 contributions, LSE to 1e-3
