@@ -613,6 +613,7 @@ def run_ours(args):
             "scaling": "strong" if args.shard == "heads" else "weak",
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": (f"BASELINE.json configs[{args.config - 1}]: {w.name}" if args.config <= 5 else
+                                    f"head_dim 64 context (not a BASELINE config): {w.name}" if args.config == 64 else
                                     f"paper Table 2 shape (context, not a BASELINE config): {w.name}"), "n_tokens": N,
                        "n_chunks": w.n_chunks, "n_docs": len(w.doc_lens), "n_q_heads": Hq, "n_kv_heads": Hkv,
                        "head_dim": d, "cu_seqlens_sha256": w.sha256(), "useful_pairs": pairs,
@@ -635,6 +636,10 @@ def run_ours(args):
             "kernels": kernels,
             "cpu_baseline": {"value": cfl / cdt / 1e12, "unit": UNIT, "cores": cthreads, "kind": "oracle",
                              "sample": cdesc, "seconds": cdt,
+                             # not run: the sample's rate applied to the whole workload's useful FLOPs (the oracle's cost per
+                             # visible pair does not depend on the document it lies in)
+                             "extrapolated": {"full_config_seconds": (w.flops_fwd + w.flops_bwd) / (cfl / cdt),
+                                              "label": "extrapolated from the sample's rate, not measured"},
                              "cfg1_full": {"value": c1fl / c1dt / 1e12, "unit": UNIT, "seconds": c1dt, "sample": c1desc}},
             "table2_context": t2, "d64_context": d64,
             "paper_context": "HSAP Table 2 (PAPER.md:158-164): SAP attention fwd+bwd 128K/SP16 = 3333.1 ms on A100s, "
@@ -651,7 +656,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=3, help="1..5 = BASELINE.json configs[0..4]; 8192..131072 = the paper's Table 2 shape at that length (context)")
+    ap.add_argument("--config", type=int, default=3, help="1..5 = BASELINE.json configs[0..4]; 64 = head_dim 64 on configs[2]'s packing (context); 8192..131072 = the paper's Table 2 shape at that length (context)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--fwd", default="pair", choices=["pair", "single"],
                     help="forward kernel: two q-heads per CTA (default when Hq/Hkv is even) or one (diagnostic)")

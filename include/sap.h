@@ -165,6 +165,8 @@ size_t sap_workspace_bytes(const sap_plan_t* plan, int n_q_heads, int n_kv_heads
  * q-chunk items in plan order and merging the per-item partials on chip (running max / sum / O).
  * q,k,v,cu_seqlens_dev: device, read.  out: device bf16 [N,Hq,d], written.  lse: device fp32 [Hq,N], written.
  * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Asynchronous.
+ * workspace / workspace_bytes: not used (the forward needs no workspace: sap_workspace_bytes(..., SAP_PASS_FWD) = 0); kept
+ * so that the two passes have the same signature.  Pass NULL, 0.
  * With an even Hq/Hkv the launch is persistent (one CTA per SM; work items = (Q tile, pair of q-heads of a group) taken
  * in order off a device counter).  Each launch needs a counter pair of its own while it runs.  The pairs come from two
  * per-device pools of 4096 that launches take round-robin and leave zeroed: one pool for ordinary launches, one for

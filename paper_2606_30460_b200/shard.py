@@ -10,7 +10,7 @@ from __future__ import annotations
 import os
 from typing import Tuple
 
-from .workloads import Workload, make_table2_workload, make_workload
+from .workloads import Workload, make_d64_workload, make_table2_workload, make_workload
 
 
 def rank_world() -> Tuple[int, int, int]:
@@ -21,6 +21,8 @@ def rank_world() -> Tuple[int, int, int]:
 
 def rank_workload(cfg: int, rank: int) -> Workload:
     """The packed sequence rank `rank` works on: same recipe, seed = rank (weak scaling: fixed work per rank)."""
+    if cfg == 64:        # head_dim 64 on configs[2]'s packing (context runs, NEXT-4)
+        return make_d64_workload(seed=rank)
     if cfg > 5:          # 8192, 16384, ...: the paper's Table 2 shape at that length (context runs, NEXT-4)
         return make_table2_workload(cfg, seed=rank)
     return make_workload(cfg, seed=rank)

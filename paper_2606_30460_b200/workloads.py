@@ -161,10 +161,10 @@ def make_table2_workload(seq_len: int, seed: int = 0) -> Workload:
                     tuple(docs), seed)
 
 
-def make_d64_workload() -> Workload:
+def make_d64_workload(seed: int = 0) -> Workload:
     """SURVEY 8(f) NEXT-4, head_dim 64: configs[2]'s packing with 64 q-heads on 16 kv-heads of 64 (the same bytes per
     token as configs[2]).  What bench.py's `d64_context` times and tests/test_gpu_configs.py checks."""
-    w0 = make_workload(3)
+    w0 = make_workload(3, seed=seed)
     return custom_workload(w0.doc_lens, w0.n_chunks, 64, 16, 64, seed=w0.seed, name="configs[2] packing, 64/16 heads, d=64")
 
 
